@@ -1,0 +1,165 @@
+/*
+ * cfgms.h — C ABI of the B200-native CFG multi-stream audio decode head.
+ *
+ * One library call = one step of the per-step audio decode head of the SpeechLM serving
+ * pipeline of arxiv 2607.02119 (citations: PAPER.md line numbers), for a continuous batch in
+ * which every classifier-free-guidance (CFG) conditional row sits next to its unconditional
+ * companion (Paired Request Co-Scheduling):
+ *
+ *   1. head projection      l^(i) = W_H (h_t + e_i), i = 0..S-1
+ *   2. CFG merge            l~ = w l_cond + (1 - w) l_uncond   (Eq. 1)
+ *   3. sampling             temperature, top-k, Gumbel-max over Philox4x32-10 noise keyed by
+ *                           (seed, request, step, stream, token)
+ *   4. token sync + delay   same token to the companion row; delayed[row][tau][i] with
+ *                           stream i lagging i steps; PAD outside the frame range
+ *                                                                          PAPER.md:56,66,76,93
+ *   5. de-interleave        grid[q][f][i] = delayed[q][f + i][i]
+ *
+ * Everything runs in hand-written sm_100a kernels; there is no CPU fallback: cfgms_create
+ * returns CFGMS_ERR_ARCH on any other device.  All entry points return a cfgms_status, never
+ * abort and never throw.  cfgms_step and cfgms_deinterleave only enqueue work on the given
+ * stream and never synchronise (they are CUDA-graph capturable); the *_host variants copy
+ * through library-owned device staging and synchronise the stream before returning.
+ *
+ * Ownership: the library owns only what it allocates (bias, scratch logits, staging, error
+ * word).  Every user pointer is borrowed; `heads` must stay valid for the context lifetime.
+ */
+#ifndef CFGMS_H
+#define CFGMS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cfgms_ctx cfgms_ctx; /* opaque */
+
+typedef enum {
+    CFGMS_OK = 0,
+    CFGMS_ERR_ARG = 1,    /* null pointer, non-positive size, bad enum                         */
+    CFGMS_ERR_SHAPE = 2,  /* d % 8 != 0, S > 64, R > max_rows, V too large for the sampler ... */
+    CFGMS_ERR_LAYOUT = 3, /* pair_map contract violated (reported by cfgms_last_device_error)  */
+    CFGMS_ERR_CUDA = 4,   /* a CUDA runtime / driver call failed                               */
+    CFGMS_ERR_ARCH = 5,   /* device is not compute capability 10.x                             */
+    CFGMS_ERR_NOMEM = 6,
+    CFGMS_ERR_TIMEOUT = 7 /* a device-side pipeline wait gave up (reported asynchronously)     */
+} cfgms_status;
+
+typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
+
+/* cfgms_config.flags */
+#define CFGMS_CFG_PAD_TOKEN 1u /* use cfgms_config.pad_token instead of the default (= V)      */
+
+typedef struct {
+    int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
+    int32_t pad_token; /* written at inactive (step, stream) cells when CFGMS_CFG_PAD_TOKEN      */
+    uint32_t flags;
+    int32_t row_tile;  /* debug/tuning: batch rows per accumulator tile (multiple of 32,
+                          <= 256); 0 = chosen from R and the SM count                           */
+    int32_t reserved[4];
+} cfgms_config;
+
+/*
+ * cfgms_create — PAPER.md:54 (shared head W_H over S audio sub-vocabularies, stream
+ * embeddings e_i).  Builds bias[i][v] = sum_k W_i[v][k] e_i[k] once (fp32), so that the
+ * per-step contraction runs on h_t alone and e_i is never rounded into bf16 with it.
+ *   heads  : DEVICE, bf16 [S][V][d], k contiguous. BORROWED for the context lifetime.
+ *   embeds : DEVICE, bf16 [S][d]. Read during the call only.
+ *   S, d, V: streams, hidden width, tokens per codebook. Requires d % 8 == 0, 1 <= S <= 64.
+ *   cfg    : nullable.
+ * Synchronises the device once.  Errors: ARG, SHAPE, ARCH, NOMEM, CUDA.
+ */
+int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t S, int32_t d,
+                 int32_t V, const cfgms_config* cfg);
+void cfgms_destroy(cfgms_ctx* ctx);
+
+/*
+ * Arguments of one decode step.  Arrays are indexed by batch row r in [0, R).
+ * Batch layout contract (the product of paired co-scheduling): the batch is a
+ * sequence of two-row slots; a slot holds one (cond, uncond) pair — cond on the EVEN row c,
+ * pair_map[c] = c + 1, pair_map[c + 1] = c — or two unpaired rows with pair_map = -1.
+ * Per-request values (w, temp, top_k, step, req_id, n_frames) are read at the cond row of a
+ * pair or at the unpaired row; the companion row's entries are ignored.
+ */
+typedef struct {
+    const void* hidden;       /* [R][d] backbone hidden states h_t, dtype below                  */
+    int32_t hidden_dtype;     /* cfgms_dtype; CFGMS_F32 is rounded to bf16 (RNE) first           */
+    int32_t R;                /* rows in the batch, 1 <= R <= max_rows                           */
+    const int32_t* pair_map;  /* [R]                                                             */
+    const float* w;           /* [R] CFG scale of Eq. 1 (any finite value)                       */
+    const float* temp;        /* [R] temperature; 0 => greedy argmax                             */
+    const int32_t* top_k;     /* [R] <= 0 or >= V: no filter; 1: greedy; ties at the k-th value
+                                 are all kept (threshold semantics)                              */
+    uint64_t seed;            /* Philox key                                                      */
+    const int32_t* step;      /* [R] request-local decode step tau >= 0: keys the noise and the
+                                 delay pattern (stream i active iff i <= tau < n_frames + i)     */
+    const uint32_t* req_id;   /* [R] request identity for the noise; NULL => the row index       */
+    const int32_t* n_frames;  /* [R] frames F of the request; NULL => no drain phase             */
+    int32_t* tokens_out;      /* [R][S] sampled tokens; the companion row receives a copy        */
+    int32_t* delayed;         /* nullable [R][T_cap][S] delayed-layout buffer, indexed by the
+                                 cond / unpaired batch row; cell [r][tau mod T_cap][i] is written */
+    int32_t T_cap;
+    float* logits_out;        /* nullable DEBUG tap: merged pre-temperature logits fp32
+                                 [R][S][V], valid at cond / unpaired rows                        */
+} cfgms_step_args;
+
+/*
+ * cfgms_step — steps 1-4 above for one batch.  Every pointer in `args` is a DEVICE pointer.
+ * Enqueues on `cuda_stream` (a cudaStream_t, may be NULL for the default stream); does not
+ * synchronise.  Errors detected on the host: ARG, SHAPE, CUDA.  A violated pair_map contract
+ * or a pipeline time-out is detected on the device and latched in a sticky error word
+ * (cfgms_last_device_error); the offending slot's tokens are then unspecified.
+ */
+int cfgms_step(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stream);
+
+/*
+ * cfgms_step_host — same step with HOST buffers: hidden, pair_map, w, temp, top_k, step,
+ * req_id, n_frames and tokens_out are HOST pointers (pinned memory recommended); `delayed`
+ * and `logits_out` stay DEVICE pointers (per-request state lives in HBM) or NULL.  Copies the
+ * inputs host->device, runs the step, copies tokens_out device->host and synchronises the
+ * stream.  Bytes moved per call are reported by cfgms_get_info.
+ */
+int cfgms_step_host(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stream);
+
+/*
+ * cfgms_deinterleave — PAPER.md:56,68: grid[q][f][i] = delayed[q][f + i][i] for
+ * 0 <= f < T - S + 1.  delayed: DEVICE int32 [n][T][S]; grid_out: DEVICE int32
+ * [n][T - S + 1][S].  Requires T >= S >= 1; n == 0 is a no-op.  Does not synchronise.
+ */
+int cfgms_deinterleave(cfgms_ctx* ctx, const int32_t* delayed, int32_t n, int32_t T, int32_t S,
+                       int32_t* grid_out, void* cuda_stream);
+/* Same with HOST buffers (copies in, runs, copies out, synchronises). */
+int cfgms_deinterleave_host(cfgms_ctx* ctx, const int32_t* delayed, int32_t n, int32_t T, int32_t S,
+                            int32_t* grid_out, void* cuda_stream);
+
+/*
+ * cfgms_last_device_error — reads the sticky device error word (one small D2H copy that
+ * synchronises the device).  Returns CFGMS_OK or the latched status; *row_out (nullable)
+ * receives the batch row it was raised for, or -1.  The word is cleared by the call.
+ */
+int cfgms_last_device_error(cfgms_ctx* ctx, int32_t* row_out);
+
+typedef struct {
+    int32_t S, d, V, max_rows, pad_token, num_sms;
+    int32_t row_tile;              /* batch rows per accumulator tile of the last step          */
+    int32_t row_blocks;            /* row tiles per vocabulary tile of the last step            */
+    int32_t vocab_tiles;           /* ceil(S*V / 128)                                           */
+    int32_t gemm_grid;             /* CTAs of the last head-GEMM launch                         */
+    int32_t pipeline_stages;       /* TMA->MMA shared-memory ring depth of the last step        */
+    int32_t launches_last_step;    /* kernels enqueued by the last cfgms_step                   */
+    int64_t launches_total;        /* kernels enqueued since create                             */
+    int64_t h2d_bytes_last_step;   /* cfgms_step_host only                                      */
+    int64_t d2h_bytes_last_step;
+} cfgms_info;
+int cfgms_get_info(cfgms_ctx* ctx, cfgms_info* out);
+
+const char* cfgms_strerror(int status);
+/* Library build string: version, arch, compile flags. */
+const char* cfgms_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CFGMS_H */

@@ -1,0 +1,8 @@
+"""cfgms — B200-native (sm_100a) CFG multi-stream audio decode head.
+
+The product is the C-ABI library `libcfgms.so` (include/cfgms.h, sources under csrc/); this
+package is its thin Python binding.  Build it in-tree with `python -m paper_2607_02119_b200.build`.
+"""
+from .binding import (CFGMS_BF16, CFGMS_F32, CfgmsError, Context, EXPORTS, LIB_PATH, library, version)
+
+__all__ = ["Context", "CfgmsError", "library", "version", "EXPORTS", "LIB_PATH", "CFGMS_BF16", "CFGMS_F32"]

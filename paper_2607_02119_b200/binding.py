@@ -1,0 +1,237 @@
+"""Thin ctypes binding of libcfgms.so (include/cfgms.h).  Argument marshalling only: every
+step of the decode-head path runs in the library's sm_100a kernels.  torch is used for device
+buffers and streams.  There is no fallback: a missing library raises at first use."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcfgms.so")
+
+CFGMS_BF16, CFGMS_F32 = 0, 1
+CFGMS_CFG_PAD_TOKEN = 1
+
+STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
+          5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
+
+EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
+           "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
+           "cfgms_version"]
+
+
+class CfgmsError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {STATUS.get(status, status)} ({_lib().cfgms_strerror(status).decode()})")
+
+
+class cfgms_config(C.Structure):
+    _fields_ = [("max_rows", C.c_int32), ("pad_token", C.c_int32), ("flags", C.c_uint32),
+                ("row_tile", C.c_int32), ("reserved", C.c_int32 * 4)]
+
+
+class cfgms_step_args(C.Structure):
+    _fields_ = [("hidden", C.c_void_p), ("hidden_dtype", C.c_int32), ("R", C.c_int32),
+                ("pair_map", C.c_void_p), ("w", C.c_void_p), ("temp", C.c_void_p), ("top_k", C.c_void_p),
+                ("seed", C.c_uint64), ("step", C.c_void_p), ("req_id", C.c_void_p), ("n_frames", C.c_void_p),
+                ("tokens_out", C.c_void_p), ("delayed", C.c_void_p), ("T_cap", C.c_int32),
+                ("logits_out", C.c_void_p)]
+
+
+class cfgms_info(C.Structure):
+    _fields_ = [("S", C.c_int32), ("d", C.c_int32), ("V", C.c_int32), ("max_rows", C.c_int32),
+                ("pad_token", C.c_int32), ("num_sms", C.c_int32), ("row_tile", C.c_int32),
+                ("row_blocks", C.c_int32), ("vocab_tiles", C.c_int32), ("gemm_grid", C.c_int32),
+                ("pipeline_stages", C.c_int32), ("launches_last_step", C.c_int32),
+                ("launches_total", C.c_int64), ("h2d_bytes_last_step", C.c_int64),
+                ("d2h_bytes_last_step", C.c_int64)]
+
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with "
+                               "`python -m paper_2607_02119_b200.build` (there is no fallback path)")
+        L = C.CDLL(LIB_PATH)
+        L.cfgms_create.restype = C.c_int
+        L.cfgms_create.argtypes = [C.POINTER(C.c_void_p), C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
+                                   C.POINTER(cfgms_config)]
+        L.cfgms_destroy.restype = None
+        L.cfgms_destroy.argtypes = [C.c_void_p]
+        for name in ("cfgms_step", "cfgms_step_host"):
+            f = getattr(L, name)
+            f.restype = C.c_int
+            f.argtypes = [C.c_void_p, C.POINTER(cfgms_step_args), C.c_void_p]
+        for name in ("cfgms_deinterleave", "cfgms_deinterleave_host"):
+            f = getattr(L, name)
+            f.restype = C.c_int
+            f.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+        L.cfgms_last_device_error.restype = C.c_int
+        L.cfgms_last_device_error.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.cfgms_get_info.restype = C.c_int
+        L.cfgms_get_info.argtypes = [C.c_void_p, C.POINTER(cfgms_info)]
+        L.cfgms_strerror.restype = C.c_char_p
+        L.cfgms_strerror.argtypes = [C.c_int]
+        L.cfgms_version.restype = C.c_char_p
+        _LIB = L
+    return _LIB
+
+
+def library():
+    """The loaded ctypes library (raises if libcfgms.so has not been built)."""
+    return _lib()
+
+
+def version() -> str:
+    return _lib().cfgms_version().decode()
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> int:
+    return (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+
+
+def _check(t: Optional[torch.Tensor], name: str, dtype, device_type: str, numel: Optional[int] = None,
+           optional: bool = False):
+    if t is None:
+        if optional:
+            return
+        raise ValueError(f"{name} is required")
+    if t.dtype not in (dtype if isinstance(dtype, tuple) else (dtype,)):
+        raise TypeError(f"{name}: expected {dtype}, got {t.dtype}")
+    if t.device.type != device_type:
+        raise ValueError(f"{name}: expected a {device_type} tensor, got {t.device}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if numel is not None and t.numel() < numel:
+        raise ValueError(f"{name}: needs at least {numel} elements, has {t.numel()}")
+
+
+class Context:
+    """cfgms_create / cfgms_destroy.  `heads` (bf16 [S][V][d], cuda) is borrowed: kept alive here."""
+
+    def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
+                 pad_token: Optional[int] = None, row_tile: int = 0):
+        _check(heads, "heads", torch.bfloat16, "cuda")
+        _check(embeds, "embeds", torch.bfloat16, "cuda")
+        if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
+            raise ValueError("heads must be [S][V][d] and embeds [S][d]")
+        self.S, self.V, self.d = (int(x) for x in heads.shape)
+        self._heads = heads
+        cfg = cfgms_config()
+        cfg.max_rows = int(max_rows)
+        cfg.row_tile = int(row_tile)
+        if pad_token is not None:
+            cfg.pad_token = int(pad_token)
+            cfg.flags = CFGMS_CFG_PAD_TOKEN
+        self.pad_token = self.V if pad_token is None else int(pad_token)
+        h = C.c_void_p()
+        with torch.cuda.device(heads.device):
+            rc = _lib().cfgms_create(C.byref(h), heads.data_ptr(), embeds.data_ptr(), self.S, self.d, self.V,
+                                     C.byref(cfg))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_create")
+        self._h = h
+        self.device = heads.device
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib().cfgms_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _args(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
+              logits_out, dev: str) -> cfgms_step_args:
+        R = int(hidden.shape[0])
+        _check(hidden, "hidden", (torch.bfloat16, torch.float32), dev, R * self.d)
+        if hidden.dim() != 2 or hidden.shape[1] != self.d:
+            raise ValueError("hidden must be [R][d]")
+        _check(pair_map, "pair_map", torch.int32, dev, R)
+        _check(w, "w", torch.float32, dev, R)
+        _check(temp, "temp", torch.float32, dev, R)
+        _check(top_k, "top_k", torch.int32, dev, R)
+        _check(step, "step", torch.int32, dev, R)
+        _check(req_id, "req_id", torch.int32, dev, R, optional=True)
+        _check(n_frames, "n_frames", torch.int32, dev, R, optional=True)
+        _check(tokens_out, "tokens_out", torch.int32, dev, R * self.S)
+        _check(delayed, "delayed", torch.int32, "cuda", optional=True)
+        _check(logits_out, "logits_out", torch.float32, "cuda", R * self.S * self.V, optional=True)
+        a = cfgms_step_args()
+        a.hidden = hidden.data_ptr()
+        a.hidden_dtype = CFGMS_F32 if hidden.dtype == torch.float32 else CFGMS_BF16
+        a.R = R
+        a.pair_map, a.w, a.temp, a.top_k = pair_map.data_ptr(), w.data_ptr(), temp.data_ptr(), top_k.data_ptr()
+        a.seed = int(seed) & 0xFFFFFFFFFFFFFFFF
+        a.step = step.data_ptr()
+        a.req_id, a.n_frames = _ptr(req_id), _ptr(n_frames)
+        a.tokens_out = tokens_out.data_ptr()
+        if delayed is not None:
+            if delayed.dim() != 3 or delayed.shape[0] < R or delayed.shape[2] != self.S:
+                raise ValueError("delayed must be [>=R][T_cap][S]")
+            a.delayed = delayed.data_ptr()
+            a.T_cap = int(delayed.shape[1])
+        a.logits_out = _ptr(logits_out)
+        return a
+
+    def step(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
+             delayed=None, logits_out=None, stream=None) -> None:
+        """cfgms_step: device tensors, enqueue only."""
+        a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
+                       logits_out, "cuda")
+        rc = _lib().cfgms_step(self._h, C.byref(a), _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_step")
+
+    def step_host(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
+                  delayed=None, logits_out=None, stream=None) -> None:
+        """cfgms_step_host: host tensors in, host tokens out; synchronises the stream."""
+        a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
+                       logits_out, "cpu")
+        rc = _lib().cfgms_step_host(self._h, C.byref(a), _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_step_host")
+
+    def deinterleave(self, delayed: torch.Tensor, grid_out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """cfgms_deinterleave(_host): [n][T][S] int32 -> [n][T-S+1][S]; host path if `delayed` is on the CPU."""
+        dev = delayed.device.type
+        _check(delayed, "delayed", torch.int32, dev)
+        if delayed.dim() != 3:
+            raise ValueError("delayed must be [n][T][S]")
+        n, T, S = (int(x) for x in delayed.shape)
+        if grid_out is None:
+            grid_out = torch.empty((n, max(T - S + 1, 0), S), dtype=torch.int32, device=delayed.device)
+        _check(grid_out, "grid_out", torch.int32, dev, n * max(T - S + 1, 0) * S)
+        fn = _lib().cfgms_deinterleave if dev == "cuda" else _lib().cfgms_deinterleave_host
+        rc = fn(self._h, delayed.data_ptr(), n, T, S, grid_out.data_ptr(), _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_deinterleave")
+        return grid_out
+
+    def last_device_error(self):
+        """-> (status, row); clears the sticky word; synchronises."""
+        row = C.c_int32(-1)
+        rc = _lib().cfgms_last_device_error(self._h, C.byref(row))
+        return rc, int(row.value)
+
+    def info(self) -> dict:
+        inf = cfgms_info()
+        rc = _lib().cfgms_get_info(self._h, C.byref(inf))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_get_info")
+        return {name: int(getattr(inf, name)) for name, _ in cfgms_info._fields_}

@@ -1,0 +1,401 @@
+// Host side of libcfgms.so: the C ABI declared in include/cfgms.h.  Validation, TMA tensor-map
+// encoding, tile-shape choice, launches.  No torch types, no CPU fallback.
+#include "../../include/cfgms.h"
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "aux_kernels.cuh"
+#include "finalize.cuh"
+#include "head_gemm.cuh"
+
+using namespace cfgms;
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct HostStage {  // device staging for the *_host entry points
+    void* hidden = nullptr;
+    int32_t *pair_map = nullptr, *top_k = nullptr, *step = nullptr, *n_frames = nullptr, *tokens = nullptr;
+    float *w = nullptr, *temp = nullptr;
+    uint32_t* req_id = nullptr;
+    int32_t* deint_in = nullptr;
+    int32_t* deint_out = nullptr;
+    size_t deint_in_bytes = 0, deint_out_bytes = 0;
+};
+
+}  // namespace
+
+struct cfgms_ctx {
+    int S = 0, d = 0, V = 0, NT = 0;
+    int device = 0, num_sms = 0;
+    int max_rows = 0, pad_token = 0, row_tile_override = 0;
+    const __nv_bfloat16* heads = nullptr;
+    float* bias = nullptr;            // [NT]
+    float* z = nullptr;               // [max_rows][NT]
+    __nv_bfloat16* hidden_bf16 = nullptr;  // [max_rows][d], used when the caller passes fp32
+    int* err = nullptr;               // device: sticky {code | row << 8}
+    EncodeTiledFn encode = nullptr;
+    CUtensorMap tmap_w;
+    CUtensorMap tmap_h;
+    const void* tmap_h_ptr = nullptr;
+    int tmap_h_R = 0, tmap_h_BN = 0;
+    int max_smem_optin = 0;
+    HostStage hs;
+    bool hs_ready = false;
+    cfgms_info info;
+};
+
+namespace {
+
+int make_tmap_2d(cfgms_ctx* c, CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    // bf16 [rows][cols], cols contiguous; box = [box_rows][64] -> 128-byte swizzled smem rows
+    cuuint64_t gdim[2] = {cols, rows};
+    cuuint64_t gstride[1] = {cols * 2};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(kBK), box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = c->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? CFGMS_OK : CFGMS_ERR_CUDA;
+}
+
+// Batch rows per accumulator tile: as few row blocks as TMEM allows (N <= 256 per MMA, two
+// accumulator stages in 512 columns), each a multiple of 32 columns so that a pair never
+// straddles a tile and tcgen05.ld.x32 chunks are whole.
+void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb) {
+    if (c->row_tile_override > 0) {
+        *BN = c->row_tile_override;
+        *nrb = (R + *BN - 1) / *BN;
+        return;
+    }
+    int blocks = (R + kMaxBN - 1) / kMaxBN;
+    int per = (R + blocks - 1) / blocks;
+    per = ((per + 31) / 32) * 32;
+    *BN = per;
+    *nrb = (R + per - 1) / per;
+}
+
+template <typename T>
+int dev_alloc(T** p, size_t n) {
+    return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T)) == cudaSuccess ? CFGMS_OK : CFGMS_ERR_NOMEM;
+}
+
+int validate_step(const cfgms_ctx* c, const cfgms_step_args* a) {
+    if (!c || !a) return CFGMS_ERR_ARG;
+    if (!a->hidden || !a->pair_map || !a->w || !a->temp || !a->top_k || !a->step || !a->tokens_out) return CFGMS_ERR_ARG;
+    if (a->hidden_dtype != CFGMS_BF16 && a->hidden_dtype != CFGMS_F32) return CFGMS_ERR_ARG;
+    if (a->R < 1) return CFGMS_ERR_ARG;
+    if (a->R > c->max_rows) return CFGMS_ERR_SHAPE;
+    if (a->delayed && a->T_cap < 1) return CFGMS_ERR_ARG;
+    return CFGMS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* cfgms_strerror(int s) {
+    switch (s) {
+        case CFGMS_OK: return "ok";
+        case CFGMS_ERR_ARG: return "invalid argument";
+        case CFGMS_ERR_SHAPE: return "unsupported shape";
+        case CFGMS_ERR_LAYOUT: return "pair_map violates the paired-slot layout contract";
+        case CFGMS_ERR_CUDA: return "CUDA call failed";
+        case CFGMS_ERR_ARCH: return "device is not sm_100 (no fallback path exists)";
+        case CFGMS_ERR_NOMEM: return "out of device memory";
+        case CFGMS_ERR_TIMEOUT: return "device-side pipeline wait timed out";
+        default: return "unknown status";
+    }
+}
+
+const char* cfgms_version(void) { return "cfgms 0.1 sm_100a (tcgen05/TMEM/TMA), built " __DATE__; }
+
+int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t S, int32_t d, int32_t V,
+                 const cfgms_config* cfg) {
+    if (!out) return CFGMS_ERR_ARG;
+    *out = nullptr;
+    if (!heads || !embeds || S < 1 || d < 1 || V < 1) return CFGMS_ERR_ARG;
+    if (S > 64 || (d % 8) != 0) return CFGMS_ERR_SHAPE;
+    if (static_cast<int64_t>(S) * V > (1ll << 30)) return CFGMS_ERR_SHAPE;
+    if ((reinterpret_cast<uintptr_t>(heads) & 15u) != 0) return CFGMS_ERR_ARG;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return CFGMS_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return CFGMS_ERR_CUDA;
+    if (prop.major != 10) return CFGMS_ERR_ARCH;
+
+    cfgms_ctx* c = new (std::nothrow) cfgms_ctx();
+    if (!c) return CFGMS_ERR_NOMEM;
+    c->S = S; c->d = d; c->V = V; c->NT = S * V;
+    c->device = dev;
+    c->num_sms = prop.multiProcessorCount;
+    c->max_smem_optin = static_cast<int>(prop.sharedMemPerBlockOptin);
+    c->max_rows = (cfg && cfg->max_rows > 0) ? cfg->max_rows : 1024;
+    c->pad_token = (cfg && (cfg->flags & CFGMS_CFG_PAD_TOKEN)) ? cfg->pad_token : V;
+    c->row_tile_override = cfg ? cfg->row_tile : 0;
+    if (c->row_tile_override < 0 || c->row_tile_override > kMaxBN || (c->row_tile_override % 32) != 0) {
+        delete c;
+        return CFGMS_ERR_ARG;
+    }
+    c->heads = static_cast<const __nv_bfloat16*>(heads);
+    std::memset(&c->info, 0, sizeof(c->info));
+
+    // the sampler keeps one row of V keys in shared memory
+    if (static_cast<size_t>(V) * 4 + 4096 > static_cast<size_t>(c->max_smem_optin)) { delete c; return CFGMS_ERR_SHAPE; }
+
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+        delete c;
+        return CFGMS_ERR_CUDA;
+    }
+    c->encode = reinterpret_cast<EncodeTiledFn>(fn);
+
+    int rc = CFGMS_OK;
+    if ((rc = dev_alloc(&c->bias, static_cast<size_t>(c->NT))) != CFGMS_OK ||
+        (rc = dev_alloc(&c->z, static_cast<size_t>(c->max_rows) * c->NT)) != CFGMS_OK ||
+        (rc = dev_alloc(&c->hidden_bf16, static_cast<size_t>(c->max_rows) * d)) != CFGMS_OK ||
+        (rc = dev_alloc(&c->err, 2)) != CFGMS_OK) {
+        cfgms_destroy(c);
+        return rc;
+    }
+    cudaMemset(c->err, 0, 2 * sizeof(int));
+
+    if ((rc = make_tmap_2d(c, &c->tmap_w, heads, static_cast<uint64_t>(c->NT), static_cast<uint64_t>(d), kBM)) != CFGMS_OK) {
+        cfgms_destroy(c);
+        return rc;
+    }
+
+    // K4: bias[i][v] = sum_k W_i[v][k] e_i[k]
+    {
+        const int warps_per_block = 8;
+        const int blocks = (c->NT + warps_per_block - 1) / warps_per_block;
+        cfgms_bias_init_kernel<<<blocks, warps_per_block * 32>>>(c->heads, static_cast<const __nv_bfloat16*>(embeds),
+                                                                  c->bias, S, V, d);
+        if (cudaDeviceSynchronize() != cudaSuccess) {
+            cfgms_destroy(c);
+            return CFGMS_ERR_CUDA;
+        }
+    }
+    const int max_gemm_smem = static_cast<int>(GemmSmemLayout::total(kMaxBN, 4));
+    if (cudaFuncSetAttribute(cfgms_head_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             c->max_smem_optin) != cudaSuccess ||
+        cudaFuncSetAttribute(cfgms_head_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             c->max_smem_optin) != cudaSuccess ||
+        max_gemm_smem > c->max_smem_optin) {
+        cfgms_destroy(c);
+        return CFGMS_ERR_CUDA;
+    }
+    if (static_cast<size_t>(V) * 4 > 40000) {
+        if (cudaFuncSetAttribute(cfgms_finalize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 static_cast<int>(static_cast<size_t>(V) * 4)) != cudaSuccess) {
+            cfgms_destroy(c);
+            return CFGMS_ERR_CUDA;
+        }
+    }
+    cudaFuncSetAttribute(cfgms_deinterleave_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+
+    c->info.S = S; c->info.d = d; c->info.V = V; c->info.max_rows = c->max_rows;
+    c->info.pad_token = c->pad_token; c->info.num_sms = c->num_sms;
+    c->info.vocab_tiles = (c->NT + kBM - 1) / kBM;
+    *out = c;
+    return CFGMS_OK;
+}
+
+void cfgms_destroy(cfgms_ctx* c) {
+    if (!c) return;
+    cudaFree(c->bias);
+    cudaFree(c->z);
+    cudaFree(c->hidden_bf16);
+    cudaFree(c->err);
+    HostStage& h = c->hs;
+    cudaFree(h.hidden); cudaFree(h.pair_map); cudaFree(h.top_k); cudaFree(h.step); cudaFree(h.n_frames);
+    cudaFree(h.tokens); cudaFree(h.w); cudaFree(h.temp); cudaFree(h.req_id); cudaFree(h.deint_in); cudaFree(h.deint_out);
+    delete c;
+}
+
+int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
+    int rc = validate_step(c, a);
+    if (rc != CFGMS_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0;
+
+    // K5: fp32 hidden -> bf16 (RNE)
+    const __nv_bfloat16* hidden = static_cast<const __nv_bfloat16*>(a->hidden);
+    if (a->hidden_dtype == CFGMS_F32) {
+        const size_t n = static_cast<size_t>(a->R) * c->d;
+        if ((reinterpret_cast<uintptr_t>(a->hidden) & 15u) != 0) return CFGMS_ERR_ARG;
+        const int blocks = static_cast<int>(std::min<size_t>((n / 4 + 255) / 256 + 1, static_cast<size_t>(c->num_sms) * 8));
+        cfgms_cast_f32_bf16_kernel<<<blocks, 256, 0, st>>>(static_cast<const float*>(a->hidden), c->hidden_bf16, n);
+        hidden = c->hidden_bf16;
+        ++launches;
+    }
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15u) != 0) return CFGMS_ERR_ARG;
+
+    int BN, nrb;
+    choose_row_tile(c, a->R, &BN, &nrb);
+    if (c->tmap_h_ptr != hidden || c->tmap_h_R != a->R || c->tmap_h_BN != BN) {
+        rc = make_tmap_2d(c, &c->tmap_h, hidden, static_cast<uint64_t>(a->R), static_cast<uint64_t>(c->d),
+                          static_cast<uint32_t>(BN));
+        if (rc != CFGMS_OK) return rc;
+        c->tmap_h_ptr = hidden; c->tmap_h_R = a->R; c->tmap_h_BN = BN;
+    }
+
+    GemmParams gp;
+    gp.R = a->R; gp.NT = c->NT; gp.d = c->d; gp.BN = BN;
+    gp.num_row_blocks = nrb;
+    gp.num_vocab_tiles = (c->NT + kBM - 1) / kBM;
+    gp.num_tiles = gp.num_vocab_tiles * nrb;
+    gp.num_kb = (c->d + kBK - 1) / kBK;
+    const uint32_t stage_bytes = GemmSmemLayout::a_bytes() + GemmSmemLayout::b_bytes(BN);
+    int stages = static_cast<int>((static_cast<uint32_t>(c->max_smem_optin) - 1024 - GemmSmemLayout::misc_bytes()) / stage_bytes);
+    stages = std::max(2, std::min(stages, kMaxStages));
+    gp.stages = stages;
+    gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp;
+    gp.bias = c->bias; gp.z = c->z; gp.tap = a->logits_out; gp.err = c->err;
+    // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
+    gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
+    gp.policy_h = kEvictLast;
+    const int grid = std::min(gp.num_tiles, c->num_sms);
+    const size_t smem = GemmSmemLayout::total(BN, stages);
+    if (a->logits_out)
+        cfgms_head_gemm_kernel<true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+    else
+        cfgms_head_gemm_kernel<false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+    ++launches;
+
+    FinalizeParams fp;
+    fp.R = a->R; fp.S = c->S; fp.V = c->V; fp.NT = c->NT;
+    fp.z = c->z; fp.pair_map = a->pair_map; fp.temp = a->temp; fp.top_k = a->top_k; fp.step = a->step;
+    fp.req_id = a->req_id; fp.n_frames = a->n_frames;
+    fp.seed_lo = static_cast<uint32_t>(a->seed & 0xffffffffull);
+    fp.seed_hi = static_cast<uint32_t>(a->seed >> 32);
+    fp.pad_token = c->pad_token;
+    fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
+    cfgms_finalize_kernel<<<dim3(c->S, a->R), kFinThreads, static_cast<size_t>(c->V) * 4, st>>>(fp);
+    ++launches;
+
+    if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
+    c->info.launches_last_step = launches;
+    c->info.launches_total += launches;
+    c->info.h2d_bytes_last_step = 0; c->info.d2h_bytes_last_step = 0;
+    return CFGMS_OK;
+}
+
+int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
+    int rc = validate_step(c, a);
+    if (rc != CFGMS_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    HostStage& h = c->hs;
+    if (!c->hs_ready) {
+        const size_t R = static_cast<size_t>(c->max_rows);
+        if (cudaMalloc(&h.hidden, R * c->d * 4) != cudaSuccess) return CFGMS_ERR_NOMEM;
+        if (dev_alloc(&h.pair_map, R) || dev_alloc(&h.top_k, R) || dev_alloc(&h.step, R) || dev_alloc(&h.n_frames, R) ||
+            dev_alloc(&h.tokens, R * c->S) || dev_alloc(&h.w, R) || dev_alloc(&h.temp, R) || dev_alloc(&h.req_id, R))
+            return CFGMS_ERR_NOMEM;
+        c->hs_ready = true;
+    }
+    const size_t R = static_cast<size_t>(a->R);
+    const size_t hid_bytes = R * c->d * (a->hidden_dtype == CFGMS_F32 ? 4 : 2);
+    int64_t h2d = 0;
+    auto up = [&](void* dst, const void* src, size_t bytes) {
+        h2d += static_cast<int64_t>(bytes);
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    };
+    bool ok = up(h.hidden, a->hidden, hid_bytes) && up(h.pair_map, a->pair_map, R * 4) && up(h.w, a->w, R * 4) &&
+              up(h.temp, a->temp, R * 4) && up(h.top_k, a->top_k, R * 4) && up(h.step, a->step, R * 4);
+    if (ok && a->req_id) ok = up(h.req_id, a->req_id, R * 4);
+    if (ok && a->n_frames) ok = up(h.n_frames, a->n_frames, R * 4);
+    if (!ok) return CFGMS_ERR_CUDA;
+    cfgms_step_args d = *a;
+    d.hidden = h.hidden; d.pair_map = h.pair_map; d.w = h.w; d.temp = h.temp; d.top_k = h.top_k; d.step = h.step;
+    d.req_id = a->req_id ? h.req_id : nullptr;
+    d.n_frames = a->n_frames ? h.n_frames : nullptr;
+    d.tokens_out = h.tokens;
+    rc = cfgms_step(c, &d, cuda_stream);
+    if (rc != CFGMS_OK) return rc;
+    const size_t tok_bytes = R * c->S * 4;
+    if (cudaMemcpyAsync(a->tokens_out, h.tokens, tok_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.h2d_bytes_last_step = h2d;
+    c->info.d2h_bytes_last_step = static_cast<int64_t>(tok_bytes);
+    return CFGMS_OK;
+}
+
+int cfgms_deinterleave(cfgms_ctx* c, const int32_t* delayed, int32_t n, int32_t T, int32_t S, int32_t* grid_out,
+                       void* cuda_stream) {
+    if (!c || n < 0 || S < 1 || T < S) return CFGMS_ERR_ARG;
+    if (n == 0) return CFGMS_OK;
+    if (!delayed || !grid_out) return CFGMS_ERR_ARG;
+    if (S > 64 || n > 65535) return CFGMS_ERR_SHAPE;
+    if ((reinterpret_cast<uintptr_t>(delayed) & 15u) != 0 || (reinterpret_cast<uintptr_t>(grid_out) & 15u) != 0)
+        return CFGMS_ERR_ARG;
+    const int F = T - S + 1;
+    const dim3 grid((F + kDeintFrames - 1) / kDeintFrames, n);
+    const size_t smem = static_cast<size_t>(kDeintFrames + S - 1) * S * 4;
+    cfgms_deinterleave_kernel<<<grid, kDeintThreads, smem, static_cast<cudaStream_t>(cuda_stream)>>>(delayed, grid_out, T, S);
+    if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.launches_total += 1;
+    return CFGMS_OK;
+}
+
+int cfgms_deinterleave_host(cfgms_ctx* c, const int32_t* delayed, int32_t n, int32_t T, int32_t S, int32_t* grid_out,
+                            void* cuda_stream) {
+    if (!c || n < 0 || S < 1 || T < S) return CFGMS_ERR_ARG;
+    if (n == 0) return CFGMS_OK;
+    if (!delayed || !grid_out) return CFGMS_ERR_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    HostStage& h = c->hs;
+    const size_t in_bytes = static_cast<size_t>(n) * T * S * 4;
+    const size_t out_bytes = static_cast<size_t>(n) * (T - S + 1) * S * 4;
+    if (in_bytes > h.deint_in_bytes) {
+        cudaFree(h.deint_in);
+        h.deint_in = nullptr; h.deint_in_bytes = 0;
+        if (cudaMalloc(reinterpret_cast<void**>(&h.deint_in), in_bytes) != cudaSuccess) return CFGMS_ERR_NOMEM;
+        h.deint_in_bytes = in_bytes;
+    }
+    if (out_bytes > h.deint_out_bytes) {
+        cudaFree(h.deint_out);
+        h.deint_out = nullptr; h.deint_out_bytes = 0;
+        if (cudaMalloc(reinterpret_cast<void**>(&h.deint_out), out_bytes) != cudaSuccess) return CFGMS_ERR_NOMEM;
+        h.deint_out_bytes = out_bytes;
+    }
+    if (cudaMemcpyAsync(h.deint_in, delayed, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    int rc = cfgms_deinterleave(c, h.deint_in, n, T, S, h.deint_out, cuda_stream);
+    if (rc != CFGMS_OK) return rc;
+    if (cudaMemcpyAsync(grid_out, h.deint_out, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    return CFGMS_OK;
+}
+
+int cfgms_last_device_error(cfgms_ctx* c, int32_t* row_out) {
+    if (!c) return CFGMS_ERR_ARG;
+    int word[2] = {0, 0};
+    cudaError_t e = cudaMemcpy(word, c->err, sizeof(word), cudaMemcpyDeviceToHost);
+    if (row_out) *row_out = -1;
+    if (e != cudaSuccess) return CFGMS_ERR_CUDA;
+    if (word[0] == 0) return CFGMS_OK;
+    if (row_out) *row_out = word[0] >> 8;
+    cudaMemset(c->err, 0, sizeof(word));
+    return word[0] & 0xff;
+}
+
+int cfgms_get_info(cfgms_ctx* c, cfgms_info* out) {
+    if (!c || !out) return CFGMS_ERR_ARG;
+    *out = c->info;
+    return CFGMS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,131 @@
+"""Shared helpers of the GPU parity tests: run the CUDA path through the C ABI on a seeded
+workload and compare it, cell by cell, with the fp64 oracle.
+
+Acceptance (BASELINE.json north_star, written here as the test's tolerance):
+  * merged pre-temperature logits: max |gpu - oracle| <= 2e-2 (fp32 accumulate of bf16)
+  * sampled token identical wherever the oracle's best-minus-second perturbed score > 2e-2
+    and the outcome does not hinge on the top-k edge within 2e-2; closer ties are counted and
+    reported, not failed
+  * PAD cells, the companion row's copy, the delayed buffer and the de-interleaved grid:
+    bit-exact
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import oracle
+import workloads
+
+LOGIT_TOL = 2e-2
+
+
+class DeviceWorkload:
+    def __init__(self, wl: workloads.Workload, dev, T_cap=None, row_tile: int = 0):
+        import paper_2607_02119_b200 as pkg
+        self.wl = wl
+        self.dev = dev
+        cu = lambda t: None if t is None else t.to(dev)
+        self.heads = cu(wl.heads)
+        self.embeds = cu(wl.embeds)
+        self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), row_tile=row_tile)
+        self.pool = cu(wl.hidden_pool)
+        self.pair_map, self.w, self.temp, self.top_k = cu(wl.pair_map), cu(wl.w), cu(wl.temp), cu(wl.top_k)
+        self.req_id, self.n_frames = cu(wl.req_id), cu(wl.n_frames)
+        self.T_cap = wl.T if T_cap is None else T_cap
+        self.delayed = torch.full((wl.R, self.T_cap, wl.S), -1, dtype=torch.int32, device=dev)
+        self.tokens = torch.full((wl.R, wl.S), -1, dtype=torch.int32, device=dev)
+
+    def hidden(self, t):
+        return self.pool[t % self.pool.shape[0]]
+
+    def step(self, t, logits_out=None, tokens=None):
+        self.ctx.step(self.hidden(t), self.pair_map, self.w, self.temp, self.top_k, self.wl.seed,
+                      self.wl.step(t).to(self.dev), self.tokens if tokens is None else tokens,
+                      req_id=self.req_id, n_frames=self.n_frames, delayed=self.delayed, logits_out=logits_out)
+
+    def check_no_device_error(self):
+        torch.cuda.synchronize()
+        rc, row = self.ctx.last_device_error()
+        assert rc == 0, f"device error {rc} at row {row}"
+
+
+def oracle_step(wl, t, cells=None, want_merged=True):
+    return oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed,
+                       wl.step(t), wl.req_id, wl.n_frames, wl.pad_token, cells=cells, want_merged=want_merged,
+                       hidden_is_f32=wl.hidden_f32)
+
+
+def sample_cells(wl, n_cells, seed):
+    """Seeded subset of (request-owning row, stream) cells the oracle computes one by one."""
+    rows = wl.head_rows()
+    allc = np.asarray([(r, i) for r in rows for i in range(wl.S)], dtype=np.int32)
+    if n_cells is None or n_cells >= len(allc):
+        return allc
+    rng = np.random.default_rng(seed)
+    idx = np.sort(rng.choice(len(allc), size=n_cells, replace=False))
+    return allc[idx]
+
+
+class ParityStats:
+    def __init__(self):
+        self.n = self.n_pad = self.n_close = self.n_close_mismatch = self.n_tight_mismatch = 0
+        self.max_logit_err = 0.0
+        self.sq_err = 0.0
+        self.n_logits = 0
+        self.first_mismatch = None
+
+    def summary(self):
+        rmse = (self.sq_err / max(self.n_logits, 1)) ** 0.5
+        return (f"cells={self.n} pad={self.n_pad} close={self.n_close} close_mismatch={self.n_close_mismatch} "
+                f"max_logit_err={self.max_logit_err:.3e} logit_rmse={rmse:.3e} first_mismatch={self.first_mismatch}")
+
+
+def compare_step(dw: DeviceWorkload, t: int, cells, stats: ParityStats, check_logits=True):
+    """Run step t on the GPU and compare the listed cells with the oracle."""
+    wl = dw.wl
+    logits = None
+    if check_logits:
+        logits = torch.zeros((wl.R, wl.S, wl.V), dtype=torch.float32, device=dw.dev)
+    dw.tokens.fill_(-1)
+    dw.step(t, logits_out=logits)
+    dw.check_no_device_error()
+    got = dw.tokens.cpu().numpy()
+    ref = oracle_step(wl, t, cells=cells, want_merged=check_logits)
+    pm = wl.pair_map.numpy()
+    if check_logits:
+        rows = torch.from_numpy(ref.cells[:, 0].astype(np.int64)).to(dw.dev)
+        strs = torch.from_numpy(ref.cells[:, 1].astype(np.int64)).to(dw.dev)
+        got_logits = logits[rows, strs].cpu().numpy().astype(np.float64)
+    tau = wl.step(t).numpy()
+    for j, (c, i) in enumerate(ref.cells):
+        stats.n += 1
+        fl = int(ref.flags[j])
+        if pm[c] >= 0:
+            assert got[pm[c], i] == got[c, i], f"companion row differs at step {t} row {c} stream {i}"
+        dslot = int(tau[c]) % dw.T_cap
+        if fl & oracle.FLAG_INACTIVE:
+            stats.n_pad += 1
+            assert got[c, i] == wl.pad_token, f"PAD expected at step {t} row {c} stream {i}, got {got[c, i]}"
+            continue
+        if check_logits:
+            err = np.abs(got_logits[j] - ref.merged[j])
+            stats.max_logit_err = max(stats.max_logit_err, float(err.max()))
+            stats.sq_err += float((err ** 2).sum())
+            stats.n_logits += err.size
+            assert err.max() <= LOGIT_TOL, f"merged logits off by {err.max()} at step {t} row {c} stream {i}"
+        assert 0 <= got[c, i] < wl.V
+        if fl & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
+            stats.n_close += 1
+            if got[c, i] != ref.tok[j]:
+                stats.n_close_mismatch += 1
+                if stats.first_mismatch is None:
+                    stats.first_mismatch = (t, int(c), int(i))
+        else:
+            assert got[c, i] == ref.tok[j], (f"token mismatch at step {t} row {c} stream {i}: gpu {got[c, i]} "
+                                             f"oracle {ref.tok[j]} margin {ref.margin[j]}")
+    # the delayed buffer received exactly tokens_out at [row][tau mod T_cap]
+    dl = dw.delayed.cpu().numpy()
+    for c in wl.head_rows():
+        assert np.array_equal(dl[c, int(tau[c]) % dw.T_cap], got[c])
+    return got

@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the fp64 oracle on the same
+seeded inputs.  Full BASELINE sizes, in the launch configuration bench.py times; at the large
+configs the oracle computes a seeded sample of (request, stream) cells one by one."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads
+from parity_util import DeviceWorkload, ParityStats, compare_step, sample_cells
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dev():
+    return torch.device("cuda:0")
+
+
+def test_config1_tiny_all_steps_and_grid(dev):
+    """BASELINE configs[0]: every token and every logit of all 24 steps, then the code grid."""
+    wl = workloads.make_config(1)
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    ref_delayed = np.full((wl.R, wl.T, wl.S), -1, dtype=np.int32)
+    for t in range(wl.T):
+        compare_step(dw, t, None, stats)
+        oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, wl.step(t),
+                    wl.req_id, wl.n_frames, wl.pad_token, delayed=ref_delayed, hidden_is_f32=True)
+    print("config1:", stats.summary())
+    assert stats.n_pad == 2 * wl.S * (wl.S - 1)          # S(S-1)/2 head + tail PAD cells per request
+    heads = wl.head_rows()
+    gpu_delayed = dw.delayed.cpu().numpy()
+    if stats.n_close_mismatch == 0:
+        assert np.array_equal(gpu_delayed[heads], ref_delayed[heads])
+    grid = dw.ctx.deinterleave(dw.delayed[torch.from_numpy(heads.astype(np.int64)).to(dev)].contiguous())
+    torch.cuda.synchronize()
+    assert grid.shape == (2, wl.T - wl.S + 1, wl.S)
+    assert np.array_equal(grid.cpu().numpy(), oracle.deinterleave(gpu_delayed[heads]))
+    assert (grid.cpu().numpy() != wl.pad_token).all()
+
+
+def test_config2_mid_and_cfg_off_twin(dev):
+    """BASELINE configs[1]: 64 pairs, d=2048, S=8, V=1024 + the CFG-off twin (64 cond rows)."""
+    wl = workloads.make_config(2)
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for t in workloads.parity_steps(2, wl.T, wl.S):
+        compare_step(dw, t, None, stats)
+    print("config2:", stats.summary())
+    assert stats.n_close < 0.06 * stats.n
+    off = workloads.cfg_off_twin(wl)
+    dwo = DeviceWorkload(off, dev)
+    so = ParityStats()
+    for t in (0, 9, 130):
+        compare_step(dwo, t, None, so)
+    print("config2 cfg-off:", so.summary())
+
+
+def test_config3_7b_head_heavy_tail(dev):
+    wl = workloads.make_config(3)
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for n, t in enumerate(workloads.parity_steps(3, wl.T, wl.S)):
+        compare_step(dw, t, sample_cells(wl, 160, seed=30 + n), stats)
+    print("config3:", stats.summary())
+
+
+def test_config4_mixed_continuous_batch(dev):
+    wl = workloads.make_config(4)
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for n, t in enumerate(workloads.parity_steps(4, wl.T, wl.S)):
+        compare_step(dw, t, sample_cells(wl, 320, seed=40 + n), stats)
+    print("config4:", stats.summary())
+    assert stats.n_pad > 0          # step 0 has not-yet-started streams for low-offset rows
+
+
+def test_config5_large_batch(dev):
+    wl = workloads.make_config(5)
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for n, t in enumerate(workloads.parity_steps(5, wl.T, wl.S)):
+        compare_step(dw, t, sample_cells(wl, 160, seed=50 + n), stats)
+    print("config5:", stats.summary())
+    info = dw.ctx.info()
+    assert info["row_blocks"] == 4 and info["row_tile"] == 256
+
+
+def test_config5_full_grid_deinterleave(dev):
+    """[512][1024][16] int32 delayed buffer -> [512][1009][16] grid, bit-exact, in full."""
+    wl = workloads.make_config(1)
+    dw = DeviceWorkload(wl, dev)
+    g = torch.Generator().manual_seed(5)
+    delayed = torch.randint(0, 2049, (512, 1024, 16), generator=g, dtype=torch.int32)
+    grid = dw.ctx.deinterleave(delayed.to(dev))
+    torch.cuda.synchronize()
+    assert grid.shape == (512, 1009, 16)
+    assert np.array_equal(grid.cpu().numpy(), oracle.deinterleave(delayed.numpy()))
+
+
+@pytest.mark.parametrize("n,T,S", [(3, 9, 9), (2, 40, 9), (5, 7, 1), (1, 300, 4), (4, 513, 16), (2, 258, 3), (0, 8, 4)])
+def test_deinterleave_edge_shapes(dev, n, T, S):
+    wl = workloads.make_config(1)
+    dw = DeviceWorkload(wl, dev)
+    g = torch.Generator().manual_seed(n * 1000 + T + S)
+    delayed = torch.randint(-5, 5000, (n, T, S), generator=g, dtype=torch.int32)
+    grid = dw.ctx.deinterleave(delayed.to(dev))
+    torch.cuda.synchronize()
+    assert grid.shape == (n, T - S + 1, S)
+    if n:
+        assert np.array_equal(grid.cpu().numpy(), oracle.deinterleave(delayed.numpy()))
+        # host-buffer entry point gives the same grid
+        assert np.array_equal(dw.ctx.deinterleave(delayed).numpy(), grid.cpu().numpy())
+
+
+def _custom(pairs, singles, d, S, V, T=16, mixed=False, **kw):
+    ov = dict(pairs=pairs, singles=singles, d=d, S=S, V=V, T=T, mixed=mixed, hidden_f32=False, heavy_tail=False)
+    ov.update(kw)
+    return workloads.make_config(2 if not mixed else 4, overrides=ov)
+
+
+@pytest.mark.parametrize("case", [
+    dict(pairs=0, singles=2, d=64, S=1, V=16),            # smallest: S = 1, one vocabulary tile, ragged
+    dict(pairs=3, singles=0, d=72, S=3, V=100),           # K tail (d % 64 != 0), NT % 128 != 0
+    dict(pairs=5, singles=6, d=256, S=9, V=520, mixed=True),   # OpusLM-like 9 streams, mixed slots
+    dict(pairs=20, singles=8, d=128, S=4, V=12800),       # 400 vocabulary tiles: >2 tiles per CTA
+    dict(pairs=100, singles=0, d=512, S=2, V=640),        # R = 200 -> one 224-row tile
+    dict(pairs=150, singles=0, d=256, S=2, V=384),        # R = 300 -> two row blocks
+])
+def test_edge_shapes_full_oracle(dev, case):
+    wl = _custom(**case)
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for t in (0, 1, wl.S, wl.T - 1):
+        compare_step(dw, t, None, stats)
+    print(case, stats.summary())
+
+
+def test_row_tile_override_many_row_blocks(dev):
+    """Force 32-row accumulator tiles: 7 row blocks x 10 vocabulary tiles through the same kernel."""
+    wl = _custom(pairs=100, singles=8, d=192, S=2, V=640, mixed=True)
+    dw = DeviceWorkload(wl, dev, row_tile=32)
+    stats = ParityStats()
+    for t in (0, 5):
+        compare_step(dw, t, None, stats)
+    assert dw.ctx.info()["row_blocks"] == 7
+    # tile shape must not change any token (determinism across tilings)
+    dw2 = DeviceWorkload(wl, dev, row_tile=0)
+    dw.step(7)
+    dw2.step(7)
+    torch.cuda.synchronize()
+    assert torch.equal(dw.tokens, dw2.tokens)
+
+
+def test_odd_row_count_and_single_row(dev):
+    wl = _custom(pairs=2, singles=2, d=128, S=4, V=256)
+    # drop the last row: R = 5, last slot holds one unpaired row
+    import dataclasses
+    cut = lambda a: None if a is None else a[:5].clone()
+    wl5 = dataclasses.replace(wl, R=5, n_req=3, hidden_pool=wl.hidden_pool[:, :5].clone(), pair_map=cut(wl.pair_map),
+                              w=cut(wl.w), temp=cut(wl.temp), top_k=cut(wl.top_k), req_id=cut(wl.req_id),
+                              n_frames=cut(wl.n_frames), offset=cut(wl.offset))
+    stats = ParityStats()
+    compare_step(DeviceWorkload(wl5, dev), 6, None, stats)
+    one = lambda a: None if a is None else a[4:5].clone()
+    wl1 = dataclasses.replace(wl, R=1, n_req=1, hidden_pool=wl.hidden_pool[:, 4:5].clone(), pair_map=one(wl.pair_map),
+                              w=one(wl.w), temp=one(wl.temp), top_k=one(wl.top_k), req_id=one(wl.req_id),
+                              n_frames=one(wl.n_frames), offset=one(wl.offset))
+    s1 = ParityStats()
+    got1 = compare_step(DeviceWorkload(wl1, dev), 6, None, s1)
+    # a request alone gives the same tokens as inside the batch (counter-based noise)
+    dw5 = DeviceWorkload(wl5, dev)
+    dw5.step(6)
+    torch.cuda.synchronize()
+    assert np.array_equal(dw5.tokens.cpu().numpy()[4], got1[0])
+
+
+def test_sampler_parameter_edges(dev):
+    """top_k <= 0, top_k >= V, top_k = 1, temp = 0, w = 0, w = 1, per-row mixes."""
+    wl = _custom(pairs=8, singles=0, d=128, S=4, V=256)
+    heads = wl.head_rows()
+    tk = [0, -3, 256, 1000, 1, 50, 2, 255]
+    tp = [1.0, 0.7, 1.3, 0.9, 0.8, 0.0, 1e-4, 1.0]
+    ww = [3.0, 0.0, 1.0, 2.5, 3.0, 3.0, -1.0, 7.5]
+    for q, r in enumerate(heads):
+        wl.top_k[r] = tk[q]
+        wl.temp[r] = tp[q]
+        wl.w[r] = ww[q]
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for t in (3, 9):
+        got = compare_step(dw, t, None, stats)
+    print("sampler edges:", stats.summary())
+    # greedy rows equal the argmax of the merged logits the GPU itself reports
+    logits = torch.zeros((wl.R, wl.S, wl.V), dtype=torch.float32, device=dev)
+    dw.step(9, logits_out=logits)
+    torch.cuda.synchronize()
+    am = logits.argmax(dim=-1).cpu().numpy()
+    for q in (4, 5):
+        assert np.array_equal(dw.tokens.cpu().numpy()[heads[q]], am[heads[q]])
+
+
+def test_w1_equals_noncfg_and_tokens_independent_of_placement(dev):
+    wl = _custom(pairs=6, singles=0, d=256, S=4, V=512)
+    wl.w[:] = 1.0
+    off = workloads.cfg_off_twin(wl)
+    a, b = DeviceWorkload(wl, dev), DeviceWorkload(off, dev)
+    for t in (4, 11):
+        a.step(t)
+        b.step(t)
+        torch.cuda.synchronize()
+        assert np.array_equal(a.tokens.cpu().numpy()[wl.head_rows()], b.tokens.cpu().numpy())
+
+
+def test_ring_buffer_depth_S(dev):
+    wl = workloads.make_config(1)
+    ring = DeviceWorkload(wl, dev, T_cap=wl.S)
+    full = DeviceWorkload(wl, dev)
+    for t in range(11):
+        ring.step(t)
+        full.step(t)
+    torch.cuda.synchronize()
+    r, f = ring.delayed.cpu().numpy(), full.delayed.cpu().numpy()
+    for t in range(7, 11):
+        assert np.array_equal(r[:, t % wl.S], f[:, t])
+
+
+def test_step_host_matches_device_path(dev):
+    wl = _custom(pairs=10, singles=4, d=256, S=4, V=384, mixed=True)
+    dw = DeviceWorkload(wl, dev)
+    dw.step(5)
+    torch.cuda.synchronize()
+    tok_host = torch.full((wl.R, wl.S), -1, dtype=torch.int32).pin_memory()
+    dw.ctx.step_host(wl.hidden(5).pin_memory(), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, wl.step(5), tok_host,
+                     req_id=wl.req_id, n_frames=wl.n_frames)
+    assert torch.equal(tok_host, dw.tokens.cpu())
+    inf = dw.ctx.info()
+    assert inf["h2d_bytes_last_step"] >= wl.R * wl.d * 2 and inf["d2h_bytes_last_step"] == wl.R * wl.S * 4
+
+
+def test_errors_are_reported_not_fatal(dev):
+    import paper_2607_02119_b200 as pkg
+    wl = _custom(pairs=4, singles=0, d=128, S=2, V=128)
+    dw = DeviceWorkload(wl, dev)
+    bad = wl.pair_map.clone()
+    bad[0], bad[1] = -1, 0            # row 1 claims row 0, row 0 does not claim back
+    dw.pair_map = bad.to(dev)
+    dw.step(3)
+    torch.cuda.synchronize()
+    rc, row = dw.ctx.last_device_error()
+    assert rc == 3 and row == 0       # CFGMS_ERR_LAYOUT at the slot's even row
+    assert dw.ctx.last_device_error()[0] == 0          # sticky word cleared
+    # host-side validation
+    small = pkg.Context(dw.heads, dw.embeds, max_rows=4)
+    with pytest.raises(pkg.CfgmsError) as e:
+        small.step(dw.hidden(0), dw.pair_map, dw.w, dw.temp, dw.top_k, 0, wl.step(0).to(dev), dw.tokens)
+    assert e.value.status == 2        # CFGMS_ERR_SHAPE: R > max_rows
+    with pytest.raises(pkg.CfgmsError):
+        pkg.Context(dw.heads[:, :, :12].contiguous(), dw.embeds[:, :12].contiguous())    # d % 8 != 0
+    # the context still works after errors
+    dw.pair_map = wl.pair_map.to(dev)
+    compare_step(dw, 3, None, ParityStats())
