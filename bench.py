@@ -1,0 +1,423 @@
+#!/usr/bin/env python
+"""bench.py — CFG audio frames/sec of the decode-head hot path on N B200s of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch: head projection + CFG merge +
+sampling + token sync + delay write (cfgms_step); the timed region also contains ONE
+cfgms_deinterleave of the full [n_req][T][S] delayed buffer (the paper de-interleaves once per
+request lifetime).  The default workload is BASELINE.json configs[4]
+("large-batch stress", the config the >= 70 % roofline target is stated on); the CFG/non-CFG
+ratio is measured on configs[1] and reported in `ratio`, and the other configs appear in
+`other_configs`.  One JSON line is printed by rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cfg_audio_frames_per_sec"
+UNIT = "frames/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per head-GEMM launch from the committed
+# `ncu --set full` capture (profiles/), keyed by config; None until captured.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), tflops=float(p["bf16_tflops"]),
+                    tflops_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), source="measured")
+    # fallback stated in B200_PROFILING.md
+    return dict(hbm_gbs=6650.0, tflops=1590.0, tflops_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event reasons through NVML during the timed region."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake_slowdown"}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+class Runner:
+    """One config resident on one GPU, stepping through the C ABI."""
+
+    def __init__(self, cfg: int, dev, cfg_off: bool = False, rank: int = 0, n_ranks: int = 1):
+        import torch
+        import paper_2607_02119_b200 as pkg
+        from paper_2607_02119_b200.dist_utils import shard_request_ids
+        import workloads
+        self.torch = torch
+        wl = workloads.make_config(cfg, cfg_off=cfg_off)
+        if rank:  # every rank serves its own requests: distinct hidden states and request ids
+            g = torch.Generator().manual_seed(1000 + rank)
+            wl.hidden_pool = torch.randn(wl.hidden_pool.shape, generator=g).to(wl.hidden_pool.dtype)
+        first, _ = shard_request_ids(rank, n_ranks, wl.n_req)
+        wl.req_id = wl.req_id + first
+        self.wl, self.dev = wl, dev
+        cu = lambda t: None if t is None else t.to(dev)
+        self.heads, self.embeds = cu(wl.heads), cu(wl.embeds)
+        self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2))
+        self.pool = cu(wl.hidden_pool)
+        self.pair_map, self.w, self.temp, self.top_k = cu(wl.pair_map), cu(wl.w), cu(wl.temp), cu(wl.top_k)
+        self.req_id, self.n_frames = cu(wl.req_id), cu(wl.n_frames)
+        self.tokens = torch.zeros((wl.R, wl.S), dtype=torch.int32, device=dev)
+        self.delayed = torch.full((wl.R, wl.T, wl.S), wl.pad_token, dtype=torch.int32, device=dev)
+        self.grid = torch.zeros((wl.R, wl.T - wl.S + 1, wl.S), dtype=torch.int32, device=dev)
+        # request-local steps of every engine iteration, resident on the device
+        ts = torch.arange(wl.T, dtype=torch.int32).unsqueeze(1) + wl.offset.unsqueeze(0)
+        self.steps_dev = ts.contiguous().to(dev)
+        self.flops_per_step = 2.0 * wl.R * wl.S * wl.d * wl.V
+        # algorithmic bytes per step: weights once, hidden once, merged
+        # logits written and read once (fp32), tokens + delayed cells
+        self.bytes_per_step = (2.0 * wl.S * wl.d * wl.V + 2.0 * wl.R * wl.d + 2 * 4.0 * wl.n_req * wl.S * wl.V
+                               + 4.0 * wl.S * (wl.R + wl.n_req))
+
+    def step(self, t: int):
+        wl = self.wl
+        self.ctx.step(self.pool[t % self.pool.shape[0]], self.pair_map, self.w, self.temp, self.top_k, wl.seed,
+                      self.steps_dev[t % wl.T], self.tokens, req_id=self.req_id, n_frames=self.n_frames,
+                      delayed=self.delayed)
+
+    def deinterleave(self):
+        self.ctx.deinterleave(self.delayed, self.grid)
+
+    def capture(self, t0: int, K: int, with_deint: bool):
+        """CUDA graph of K consecutive steps (+ the de-interleave)."""
+        torch = self.torch
+        g = torch.cuda.CUDAGraph()
+        s = torch.cuda.Stream(device=self.dev)
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            self.step(t0)
+        torch.cuda.current_stream().wait_stream(s)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            for j in range(K):
+                self.step(t0 + j)
+            if with_deint:
+                self.deinterleave()
+        return g
+
+    def time_graph(self, K: int, warmup: int, with_deint: bool, barrier=None, sampler=None):
+        """-> elapsed ms of one replay of a K-step graph (after `warmup` eager steps + one replay)."""
+        torch = self.torch
+        for t in range(warmup):
+            self.step(t)
+        g = self.capture(warmup, K, with_deint)
+        g.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if barrier:
+            barrier()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.__enter__()
+        e0.record()
+        g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.__exit__()
+        if barrier:
+            barrier()
+        return e0.elapsed_time(e1)
+
+    def time_kernels(self, K: int, warmup: int):
+        """Per-kernel device time with CUDA events on the launch stream: (gemm us, finalize us) per step."""
+        torch = self.torch
+        for t in range(warmup):
+            self.step(t)
+        torch.cuda.synchronize()
+        self.ctx.profile_enable(True)
+        for j in range(K):
+            self.step(warmup + j)
+        gm, fm, n = self.ctx.profile_read()
+        self.ctx.profile_enable(False)
+        return 1e3 * gm / max(n, 1), 1e3 * fm / max(n, 1)
+
+    def time_cold(self, K: int, flush):
+        """Per-step device time with an untimed L2 flush before every step (median us)."""
+        torch = self.torch
+        times = []
+        for j in range(K):
+            flush.add_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            self.step(j)
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1) * 1e3)
+        times.sort()
+        return times[len(times) // 2]
+
+    def time_e2e(self, K: int, warmup: int):
+        """Same step through cfgms_step_host: pinned host inputs in, host tokens out, every step."""
+        torch = self.torch
+        wl = self.wl
+        pin = lambda t: None if t is None else t.contiguous().pin_memory()
+        pool = [pin(wl.hidden_pool[j]) for j in range(wl.hidden_pool.shape[0])]
+        pm, w, temp, tk, rid, nf = map(pin, (wl.pair_map, wl.w, wl.temp, wl.top_k, wl.req_id, wl.n_frames))
+        steps = [pin((wl.offset + t).to(torch.int32)) for t in range(min(wl.T, warmup + K))]
+        tok = torch.zeros((wl.R, wl.S), dtype=torch.int32).pin_memory()
+        call = lambda t: self.ctx.step_host(pool[t % len(pool)], pm, w, temp, tk, wl.seed, steps[t % len(steps)], tok,
+                                            req_id=rid, n_frames=nf, delayed=self.delayed)
+        for t in range(warmup):
+            call(t)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for j in range(K):
+            call(warmup + j)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        inf = self.ctx.info()
+        return dt, inf["h2d_bytes_last_step"], inf["d2h_bytes_last_step"]
+
+
+def oracle_sample(wl, budget_s: float = 12.0):
+    """Times the fp64 oracle, as it stands, on a bounded seeded sample of cells of one step."""
+    import numpy as np
+    import oracle
+    rows = wl.head_rows()
+    cells = np.asarray([(r, i) for r in rows for i in range(wl.S)], dtype=np.int32)
+    rng = np.random.default_rng(0)
+    rng.shuffle(cells)
+    t = wl.S  # every stream active
+    run = lambda cl: oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed,
+                                 wl.step(t), wl.req_id, wl.n_frames, wl.pad_token, cells=cl,
+                                 hidden_is_f32=wl.hidden_f32)
+    n0 = min(len(cells), 4 * oracle.num_threads())
+    t0 = time.perf_counter()
+    run(cells[:n0])
+    dt0 = time.perf_counter() - t0
+    n = int(min(len(cells), max(n0, n0 * budget_s / max(dt0, 1e-6))))
+    t0 = time.perf_counter()
+    run(cells[:n])
+    dt = time.perf_counter() - t0
+    frames = n / wl.S           # one frame = S tokens of one request
+    return dict(value=frames / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"{n} of {len(cells)} (request, stream) cells of one step of {wl.name}, {dt:.1f} s"), dt, n
+
+
+def run_reference(args):
+    """--impl reference: the oracle (fp64, CPU) on this arm's config and metric; rank 0 only.
+    Each step is a bounded seeded sample of that step's (request, stream) cells, sized so that the
+    whole --steps/--warmup run ends within about two minutes."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    import oracle
+    import workloads
+    wl = workloads.make_config(args.config)
+    rows = wl.head_rows()
+    cells = np.asarray([(r, i) for r in rows for i in range(wl.S)], dtype=np.int32)
+    np.random.default_rng(0).shuffle(cells)
+    run = lambda t, cl: oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed,
+                                    wl.step(t), wl.req_id, wl.n_frames, wl.pad_token, cells=cl,
+                                    hidden_is_f32=wl.hidden_f32)
+    threads = oracle.num_threads()
+    n0 = min(len(cells), 2 * threads)
+    t0 = time.perf_counter()
+    run(wl.S, cells[:n0])
+    rate = n0 / (time.perf_counter() - t0)                     # cells per second
+    per_step = 100.0 / max(args.steps + args.warmup, 1)
+    n = int(min(len(cells), max(threads, rate * per_step)))
+    frames = secs = 0.0
+    for j in range(args.warmup + args.steps):
+        t = wl.S + (j % (wl.T - 2 * wl.S))                       # every stream active
+        lo = (j * n) % max(len(cells) - n + 1, 1)
+        t0 = time.perf_counter()
+        run(t, cells[lo:lo + n])
+        dt = time.perf_counter() - t0
+        if j >= args.warmup:
+            frames += n / wl.S
+            secs += dt
+    value = frames / secs
+    cb = dict(value=value, unit=UNIT, cores=threads, kind="oracle",
+              sample=f"{n} of {len(cells)} (request, stream) cells per step of {wl.name}, {args.steps} steps, {secs:.1f} s")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wl.n_req / value, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(wl, args.config, "cpu oracle on a bounded sample of cells per step"),
+            "cpu_baseline": cb,
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(wl, cfg, launch):
+    return {"workload": f"BASELINE.json configs[{cfg - 1}] '{wl.name}': {wl.n_req} requests in {wl.R} rows "
+                        f"({int((wl.pair_map >= 0).sum()) // 2} CFG pairs), d={wl.d}, S={wl.S}, V={wl.V}, T={wl.T}",
+            "rows": wl.R, "requests": wl.n_req, "d": wl.d, "S": wl.S, "V": wl.V, "T": wl.T,
+            "parallelism": "request-sharded replicas (no data-path collective)", "launch": launch}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip ratio / other configs / cold-L2 legs")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    from paper_2607_02119_b200 import dist_utils
+    import paper_2607_02119_b200 as pkg
+    pkg.library()  # fail loudly before anything else if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    rank, local_rank, world = dist_utils.init("nccl")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    peaks = load_peaks()
+    K, W = args.steps, args.warmup
+
+    main_r = Runner(args.config, dev, rank=rank, n_ranks=world)
+    wl = main_r.wl
+    K = min(K, 4096)
+    sampler = ClockSampler(local_rank)
+    elapsed_ms = main_r.time_graph(K, W, with_deint=True, barrier=lambda: dist_utils.barrier(dev), sampler=sampler)
+    value, worst_ms = dist_utils.whole_job_rate(float(wl.n_req) * K, elapsed_ms, dev)
+    info = main_r.ctx.info()
+    gemm_us, fin_us = main_r.time_kernels(min(K, 512), 3)
+    us_per_step = 1e3 * worst_ms / K
+
+    line = None
+    if rank == 0:
+        t_tensor = main_r.flops_per_step / (peaks["tflops"] * 1e12)
+        t_hbm = main_r.bytes_per_step / (peaks["hbm_gbs"] * 1e9)
+        if t_tensor >= t_hbm:
+            roof = {"bound": "tensor", "achieved": main_r.flops_per_step / (gemm_us * 1e-6) / 1e12,
+                    "peak": peaks["tflops"], "unit": "TFLOP/s"}
+        else:
+            roof = {"bound": "hbm", "achieved": main_r.bytes_per_step / (gemm_us * 1e-6) / 1e9,
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+        roof["frac"] = roof["achieved"] / roof["peak"]
+        roof["traffic"] = NCU_TRAFFIC_BYTES.get(args.config)
+        roof.update(kernel="cfgms_head_gemm_kernel", kernel_us=gemm_us, finalize_us=fin_us, peak_source=peaks["source"],
+                    roofline_us_per_step=1e6 * max(t_tensor, t_hbm), step_frac=max(t_tensor, t_hbm) * 1e6 / us_per_step,
+                    frac_of_sustained_peak=(roof["achieved"] / peaks["tflops_sustained"]) if roof["bound"] == "tensor" else None)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": worst_ms / K, "us_per_step": us_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": dict(workload_config(wl, args.config, f"one CUDA graph of {K} cfgms_step + 1 cfgms_deinterleave"),
+                               l2="inputs larger than L2: head weights %.0f MiB + hidden pool %.0f MiB + logits %.0f MiB" % (
+                                   wl.heads.numel() * 2 / 2 ** 20, wl.hidden_pool.numel() * wl.hidden_pool.element_size() / 2 ** 20,
+                                   wl.n_req * wl.S * wl.V * 4 / 2 ** 20),
+                               row_tile=info["row_tile"], row_blocks=info["row_blocks"], gemm_grid=info["gemm_grid"],
+                               pipeline_stages=info["pipeline_stages"]),
+                "clocks": sampler.summary(), "gpu_launches": int(info["launches_last_step"] * K + 1), "roofline": roof}
+
+    # end-to-end through the host-buffer entry point (every rank, max over ranks)
+    Ke = min(K, 64)
+    dt_e2e, h2d, d2h = main_r.time_e2e(Ke, 3)
+    e2e_value, _ = dist_utils.whole_job_rate(float(wl.n_req) * Ke, dt_e2e * 1e3, dev)
+    if rank == 0:
+        line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                       "us_per_step": 1e6 * dt_e2e / Ke, "api": "cfgms_step_host (pinned host buffers, sync per step)"}
+
+    if rank == 0 and world == 1:
+        cb, _, _ = oracle_sample(wl)
+        line["cpu_baseline"] = cb
+        if not args.no_extras:
+            del main_r
+            torch.cuda.empty_cache()
+            flush = torch.zeros(256 * 2 ** 20 // 4, dtype=torch.int32, device=dev)
+            extras = {}
+            ratio = {}
+            for cfg in (2, 3, 4):
+                if cfg == args.config:
+                    continue
+                r = Runner(cfg, dev)
+                ms = r.time_graph(min(K, r.wl.T), W, with_deint=False)
+                hot_us = 1e3 * ms / min(K, r.wl.T)
+                g_us, f_us = r.time_kernels(64, 3)
+                cold_us = r.time_cold(48, flush)
+                t_roof = max(r.flops_per_step / (peaks["tflops"] * 1e12), r.bytes_per_step / (peaks["hbm_gbs"] * 1e9)) * 1e6
+                extras[f"config{cfg}"] = {"us_per_step_hot": hot_us, "us_per_step_cold_l2": cold_us, "gemm_us": g_us,
+                                          "finalize_us": f_us, "frames_per_s_hot": r.wl.n_req / hot_us * 1e6,
+                                          "roofline_us": t_roof, "frac_hot": t_roof / hot_us, "frac_cold": t_roof / cold_us}
+                if cfg in (2, 3):
+                    ro = Runner(cfg, dev, cfg_off=True)
+                    ms_o = ro.time_graph(min(K, ro.wl.T), W, with_deint=False)
+                    hot_o = 1e3 * ms_o / min(K, ro.wl.T)
+                    cold_o = ro.time_cold(48, flush)
+                    ratio[f"config{cfg}"] = {"cfg_us": hot_us, "noncfg_us": hot_o, "ratio_equal_requests_hot": hot_o / hot_us,
+                                             "cfg_us_cold": cold_us, "noncfg_us_cold": cold_o,
+                                             "ratio_equal_requests_cold_l2": cold_o / cold_us}
+                    del ro
+                del r
+                torch.cuda.empty_cache()
+            line["other_configs"] = extras
+            line["ratio"] = dict(ratio, paper_context="paper: CFG sustains 80% of non-CFG decode tok/s, whole engine, "
+                                                      "1x H100 80GB, equal rows (PAPER.md:154-163)")
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist_utils.barrier(dev)
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

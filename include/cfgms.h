@@ -155,6 +155,16 @@ typedef struct {
 } cfgms_info;
 int cfgms_get_info(cfgms_ctx* ctx, cfgms_info* out);
 
+/*
+ * Profiling aid (bench.py's roofline figure).  While enabled, cfgms_step records CUDA events
+ * on the launch stream before the head GEMM, between it and the finalize kernel, and after;
+ * cfgms_profile_read waits for them and returns the summed device time of each kernel and the
+ * number of recorded steps (at most 4096 between reads), then resets the ring.  Event records
+ * perturb back-to-back launches slightly: time throughput with profiling off.
+ */
+int cfgms_profile_enable(cfgms_ctx* ctx, int on);
+int cfgms_profile_read(cfgms_ctx* ctx, double* gemm_ms, double* finalize_ms, int64_t* steps);
+
 const char* cfgms_strerror(int status);
 /* Library build string: version, arch, compile flags. */
 const char* cfgms_version(void);

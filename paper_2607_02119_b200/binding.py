@@ -20,7 +20,7 @@ STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR
 
 EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
-           "cfgms_version"]
+           "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read"]
 
 
 class CfgmsError(RuntimeError):
@@ -78,6 +78,10 @@ def _lib():
         L.cfgms_last_device_error.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
         L.cfgms_get_info.restype = C.c_int
         L.cfgms_get_info.argtypes = [C.c_void_p, C.POINTER(cfgms_info)]
+        L.cfgms_profile_enable.restype = C.c_int
+        L.cfgms_profile_enable.argtypes = [C.c_void_p, C.c_int]
+        L.cfgms_profile_read.restype = C.c_int
+        L.cfgms_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cfgms_strerror.restype = C.c_char_p
         L.cfgms_strerror.argtypes = [C.c_int]
         L.cfgms_version.restype = C.c_char_p
@@ -228,6 +232,19 @@ class Context:
         row = C.c_int32(-1)
         rc = _lib().cfgms_last_device_error(self._h, C.byref(row))
         return rc, int(row.value)
+
+    def profile_enable(self, on: bool) -> None:
+        rc = _lib().cfgms_profile_enable(self._h, int(bool(on)))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_profile_enable")
+
+    def profile_read(self):
+        """-> (head-GEMM ms, finalize ms, steps) summed since the last read; synchronises."""
+        g, f, n = C.c_double(), C.c_double(), C.c_int64()
+        rc = _lib().cfgms_profile_read(self._h, C.byref(g), C.byref(f), C.byref(n))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_profile_read")
+        return float(g.value), float(f.value), int(n.value)
 
     def info(self) -> dict:
         inf = cfgms_info()

@@ -23,6 +23,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+constexpr int kProfMax = 4096;
+
 struct HostStage {  // device staging for the *_host entry points
     void* hidden = nullptr;
     int32_t *pair_map = nullptr, *top_k = nullptr, *step = nullptr, *n_frames = nullptr, *tokens = nullptr;
@@ -52,6 +54,9 @@ struct cfgms_ctx {
     int max_smem_optin = 0;
     HostStage hs;
     bool hs_ready = false;
+    bool prof_on = false;
+    cudaEvent_t* prof_ev = nullptr;   // [kProfMax][3]
+    int prof_n = 0;
     cfgms_info info;
 };
 
@@ -219,6 +224,10 @@ void cfgms_destroy(cfgms_ctx* c) {
     cudaFree(c->z);
     cudaFree(c->hidden_bf16);
     cudaFree(c->err);
+    if (c->prof_ev) {
+        for (int j = 0; j < 3 * kProfMax; ++j) cudaEventDestroy(c->prof_ev[j]);
+        delete[] c->prof_ev;
+    }
     HostStage& h = c->hs;
     cudaFree(h.hidden); cudaFree(h.pair_map); cudaFree(h.top_k); cudaFree(h.step); cudaFree(h.n_frames);
     cudaFree(h.tokens); cudaFree(h.w); cudaFree(h.temp); cudaFree(h.req_id); cudaFree(h.deint_in); cudaFree(h.deint_out);
@@ -269,11 +278,14 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     gp.policy_h = kEvictLast;
     const int grid = std::min(gp.num_tiles, c->num_sms);
     const size_t smem = GemmSmemLayout::total(BN, stages);
+    const bool prof = c->prof_on && c->prof_n < kProfMax;
+    if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
     if (a->logits_out)
         cfgms_head_gemm_kernel<true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
     else
         cfgms_head_gemm_kernel<false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
     ++launches;
+    if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 1], st);
 
     FinalizeParams fp;
     fp.R = a->R; fp.S = c->S; fp.V = c->V; fp.NT = c->NT;
@@ -285,6 +297,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
     cfgms_finalize_kernel<<<dim3(c->S, a->R), kFinThreads, static_cast<size_t>(c->V) * 4, st>>>(fp);
     ++launches;
+    if (prof) { cudaEventRecord(c->prof_ev[3 * c->prof_n + 2], st); ++c->prof_n; }
 
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
@@ -390,6 +403,36 @@ int cfgms_last_device_error(cfgms_ctx* c, int32_t* row_out) {
     if (row_out) *row_out = word[0] >> 8;
     cudaMemset(c->err, 0, sizeof(word));
     return word[0] & 0xff;
+}
+
+int cfgms_profile_enable(cfgms_ctx* c, int on) {
+    if (!c) return CFGMS_ERR_ARG;
+    if (on && !c->prof_ev) {
+        c->prof_ev = new (std::nothrow) cudaEvent_t[3 * kProfMax];
+        if (!c->prof_ev) return CFGMS_ERR_NOMEM;
+        for (int j = 0; j < 3 * kProfMax; ++j)
+            if (cudaEventCreate(&c->prof_ev[j]) != cudaSuccess) return CFGMS_ERR_CUDA;
+    }
+    c->prof_on = on != 0;
+    c->prof_n = 0;
+    return CFGMS_OK;
+}
+
+int cfgms_profile_read(cfgms_ctx* c, double* gemm_ms, double* finalize_ms, int64_t* steps) {
+    if (!c || !gemm_ms || !finalize_ms || !steps) return CFGMS_ERR_ARG;
+    double g = 0.0, f = 0.0;
+    for (int j = 0; j < c->prof_n; ++j) {
+        float a = 0.f, b = 0.f;
+        if (cudaEventSynchronize(c->prof_ev[3 * j + 2]) != cudaSuccess) return CFGMS_ERR_CUDA;
+        if (cudaEventElapsedTime(&a, c->prof_ev[3 * j], c->prof_ev[3 * j + 1]) != cudaSuccess ||
+            cudaEventElapsedTime(&b, c->prof_ev[3 * j + 1], c->prof_ev[3 * j + 2]) != cudaSuccess)
+            return CFGMS_ERR_CUDA;
+        g += a;
+        f += b;
+    }
+    *gemm_ms = g; *finalize_ms = f; *steps = c->prof_n;
+    c->prof_n = 0;
+    return CFGMS_OK;
 }
 
 int cfgms_get_info(cfgms_ctx* c, cfgms_info* out) {
