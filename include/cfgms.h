@@ -51,6 +51,9 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
 
 /* cfgms_config.flags */
 #define CFGMS_CFG_PAD_TOKEN 1u /* use cfgms_config.pad_token instead of the default (= V)      */
+#define CFGMS_CFG_NO_CANDIDATES 2u /* tuning/debug: never use the fused per-chunk candidate pass;
+                                      the sampler then scans all V logits of every cell (the path
+                                      always taken when V % 32 != 0 or V > 8192)                 */
 
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */

@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libcfgms.so")
 
 CFGMS_BF16, CFGMS_F32 = 0, 1
 CFGMS_CFG_PAD_TOKEN = 1
+CFGMS_CFG_NO_CANDIDATES = 2
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
           5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
@@ -126,7 +127,7 @@ class Context:
     """cfgms_create / cfgms_destroy.  `heads` (bf16 [S][V][d], cuda) is borrowed: kept alive here."""
 
     def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
-                 pad_token: Optional[int] = None, row_tile: int = 0):
+                 pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -138,7 +139,9 @@ class Context:
         cfg.row_tile = int(row_tile)
         if pad_token is not None:
             cfg.pad_token = int(pad_token)
-            cfg.flags = CFGMS_CFG_PAD_TOKEN
+            cfg.flags |= CFGMS_CFG_PAD_TOKEN
+        if no_candidates:
+            cfg.flags |= CFGMS_CFG_NO_CANDIDATES
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):

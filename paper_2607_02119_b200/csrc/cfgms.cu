@@ -44,6 +44,9 @@ struct cfgms_ctx {
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT]
     float* z = nullptr;               // [max_rows][NT]
+    float* cand_val = nullptr;        // [max_rows][NT/32][4] top-4 per 32-token chunk (candidate path)
+    uint32_t* cand_src = nullptr;     // [max_rows][NT/32]
+    bool use_cand = false;            // V % 32 == 0 && V <= 8192
     __nv_bfloat16* hidden_bf16 = nullptr;  // [max_rows][d], used when the caller passes fp32
     int* err = nullptr;               // device: sticky {code | row << 8}
     EncodeTiledFn encode = nullptr;
@@ -154,6 +157,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
         return CFGMS_ERR_ARG;
     }
     c->heads = static_cast<const __nv_bfloat16*>(heads);
+    c->use_cand = (V % 32 == 0) && V <= 8192 && !(cfg && (cfg->flags & CFGMS_CFG_NO_CANDIDATES));
     std::memset(&c->info, 0, sizeof(c->info));
 
     // the sampler keeps one row of V keys in shared memory
@@ -171,7 +175,9 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     if ((rc = dev_alloc(&c->bias, static_cast<size_t>(c->NT))) != CFGMS_OK ||
         (rc = dev_alloc(&c->z, static_cast<size_t>(c->max_rows) * c->NT)) != CFGMS_OK ||
         (rc = dev_alloc(&c->hidden_bf16, static_cast<size_t>(c->max_rows) * d)) != CFGMS_OK ||
-        (rc = dev_alloc(&c->err, 2)) != CFGMS_OK) {
+        (rc = dev_alloc(&c->err, 2)) != CFGMS_OK ||
+        (c->use_cand && ((rc = dev_alloc(&c->cand_val, static_cast<size_t>(c->max_rows) * (c->NT / 32) * 4)) != CFGMS_OK ||
+                         (rc = dev_alloc(&c->cand_src, static_cast<size_t>(c->max_rows) * (c->NT / 32))) != CFGMS_OK))) {
         cfgms_destroy(c);
         return rc;
     }
@@ -194,20 +200,24 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
         }
     }
     const int max_gemm_smem = static_cast<int>(GemmSmemLayout::total(kMaxBN, 4));
-    if (cudaFuncSetAttribute(cfgms_head_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (cudaFuncSetAttribute(cfgms_head_gemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              c->max_smem_optin) != cudaSuccess ||
-        cudaFuncSetAttribute(cfgms_head_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaFuncSetAttribute(cfgms_head_gemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              c->max_smem_optin) != cudaSuccess ||
+        cudaFuncSetAttribute(cfgms_head_gemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             c->max_smem_optin) != cudaSuccess ||
+        cudaFuncSetAttribute(cfgms_head_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             c->max_smem_optin) != cudaSuccess ||
+        cudaFuncSetAttribute(cfgms_finalize_cand_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
         max_gemm_smem > c->max_smem_optin) {
         cfgms_destroy(c);
         return CFGMS_ERR_CUDA;
     }
-    if (static_cast<size_t>(V) * 4 > 40000) {
-        if (cudaFuncSetAttribute(cfgms_finalize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 static_cast<int>(static_cast<size_t>(V) * 4)) != cudaSuccess) {
-            cfgms_destroy(c);
-            return CFGMS_ERR_CUDA;
-        }
+    if (cudaFuncSetAttribute(cfgms_finalize_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        (V > 256 * 32 && cudaFuncSetAttribute(cfgms_finalize_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              static_cast<int>(static_cast<size_t>(V) * 4)) != cudaSuccess)) {
+        cfgms_destroy(c);
+        return CFGMS_ERR_CUDA;
     }
     cudaFuncSetAttribute(cfgms_deinterleave_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
 
@@ -222,6 +232,8 @@ void cfgms_destroy(cfgms_ctx* c) {
     if (!c) return;
     cudaFree(c->bias);
     cudaFree(c->z);
+    cudaFree(c->cand_val);
+    cudaFree(c->cand_src);
     cudaFree(c->hidden_bf16);
     cudaFree(c->err);
     if (c->prof_ev) {
@@ -273,6 +285,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     gp.stages = stages;
     gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp;
     gp.bias = c->bias; gp.z = c->z; gp.tap = a->logits_out; gp.err = c->err;
+    gp.cand_val = c->cand_val; gp.cand_src = c->cand_src;
     // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;
@@ -280,10 +293,13 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     const size_t smem = GemmSmemLayout::total(BN, stages);
     const bool prof = c->prof_on && c->prof_n < kProfMax;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
-    if (a->logits_out)
-        cfgms_head_gemm_kernel<true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
-    else
-        cfgms_head_gemm_kernel<false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+    if (a->logits_out) {
+        if (c->use_cand) cfgms_head_gemm_kernel<true, true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+        else cfgms_head_gemm_kernel<true, false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+    } else {
+        if (c->use_cand) cfgms_head_gemm_kernel<false, true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+        else cfgms_head_gemm_kernel<false, false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+    }
     ++launches;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 1], st);
 
@@ -295,7 +311,21 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.seed_hi = static_cast<uint32_t>(a->seed >> 32);
     fp.pad_token = c->pad_token;
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
-    cfgms_finalize_kernel<<<dim3(c->S, a->R), kFinThreads, static_cast<size_t>(c->V) * 4, st>>>(fp);
+    fp.cand_val = c->cand_val; fp.cand_src = c->cand_src;
+    if (c->use_cand) {
+        const int G = c->V / 32, E = 4 * G;
+        const size_t fsmem = static_cast<size_t>(kCandWarps) * (3 * E + G + 256 + 64) * 4;
+        const int cells = a->R * c->S;
+        cfgms_finalize_cand_kernel<<<(cells + kCandWarps - 1) / kCandWarps, kCandWarps * 32, fsmem, st>>>(fp);
+    } else {
+        const dim3 fgrid(c->S, a->R);
+        const size_t fsmem = static_cast<size_t>(c->V) * 8;
+        if (c->V <= 256 * 4) cfgms_finalize_kernel<4><<<fgrid, kFinThreads, fsmem, st>>>(fp);
+        else if (c->V <= 256 * 8) cfgms_finalize_kernel<8><<<fgrid, kFinThreads, fsmem, st>>>(fp);
+        else if (c->V <= 256 * 16) cfgms_finalize_kernel<16><<<fgrid, kFinThreads, fsmem, st>>>(fp);
+        else if (c->V <= 256 * 32) cfgms_finalize_kernel<32><<<fgrid, kFinThreads, fsmem, st>>>(fp);
+        else cfgms_finalize_large_kernel<<<fgrid, kFinThreads, static_cast<size_t>(c->V) * 4, st>>>(fp);
+    }
     ++launches;
     if (prof) { cudaEventRecord(c->prof_ev[3 * c->prof_n + 2], st); ++c->prof_n; }
 

@@ -1,10 +1,18 @@
 // K2 — top-k threshold, Gumbel-max over Philox4x32-10 noise, companion token sync and the
 // delay-layout write (rows a3-a4 of DESIGN.md's hot-path table).
 //
-// One CTA per (request-owning batch row, stream).  The row's V temperature-scaled merged
-// logits z (fp32, written by K1, normally still L2-resident) are turned into order-preserving
-// 32-bit keys in shared memory; an exact 4-pass 8-bit radix select finds the k-th largest key
-// (threshold semantics: every z >= threshold survives); only the survivors draw noise.
+// One CTA of 256 threads per (request-owning batch row, stream).  The row's V temperature-
+// scaled merged logits z (fp32, written by K1, normally still L2-resident) are loaded ONCE
+// into registers as order-preserving 32-bit keys.  Exact top-k threshold without sorting V
+// values and without hammering shared-memory atomics:
+//   1. every thread takes the max of its V/256 keys; every warp extracts the ceil(k/8)-th
+//      largest of its 32 thread maxima (redux.sync loop).  The minimum L of the 8 warp values
+//      is a LOWER BOUND of the k-th largest key (at least 8*ceil(k/8) >= k keys are >= L);
+//   2. keys >= L are compacted to shared memory (about 2k candidates in practice);
+//   3. one warp runs an exact MSB-first 8-bit radix select on the candidates only;
+//   4. survivors (key >= threshold; ties kept) draw Gumbel noise; block argmax, lowest index
+//      on ties.
+// k > 256 (or V tiny) degrades gracefully: L = 0 and every key is a candidate.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -12,6 +20,7 @@
 namespace cfgms {
 
 constexpr int kFinThreads = 256;
+constexpr int kFinWarps = kFinThreads / 32;
 
 struct FinalizeParams {
     int R, S, V, NT;
@@ -27,6 +36,8 @@ struct FinalizeParams {
     int32_t* tokens_out;      // [R][S]
     int32_t* delayed;         // nullable [R][T_cap][S]
     int32_t T_cap;
+    const float* cand_val;    // [R][NT/32][4]  (candidate path only)
+    const uint32_t* cand_src; // [R][NT/32]
 };
 
 // Philox4x32-10 (Salmon et al. 2011): ten rounds of two 32x32->64 multiplies with key bumps.
@@ -53,29 +64,115 @@ __device__ __forceinline__ float gumbel_noise(uint32_t seed_lo, uint32_t seed_hi
     const int wsel = v & 3;
     const uint32_t x = wsel == 0 ? o.x : wsel == 1 ? o.y : wsel == 2 ? o.z : o.w;
     const float p = (static_cast<float>(x >> 9) + 0.5f) * 1.1920928955078125e-07f;  // 2^-23
-    return -logf(-log1pf(-p));
+    // inner log1p keeps full relative accuracy of E = -ln(1-p) for small p; the outer logarithm may be
+    // the fast one (abs. error <= 2^-21.4 near 1, <= 3 ulp elsewhere: < 1e-5 on |g| <= 17)
+    return -__logf(-log1pf(-p));
 }
 
+// Order-preserving float -> uint32 (larger float <=> larger key).  Every real key is >= 1;
+// 0 is reserved for "no element".
 __device__ __forceinline__ uint32_t float_key(float f) {
     f += 0.0f;  // -0 -> +0 so that equal floats have equal keys
     const uint32_t u = __float_as_uint(f);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    const uint32_t k = (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    return k == 0u ? 1u : k;   // only the all-ones negative NaN maps to 0
 }
 __device__ __forceinline__ float key_float(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
 
+struct BestSV {
+    float s;
+    int v;
+};
+__device__ __forceinline__ void best_update(BestSV& b, float s, int v) {
+    if (s > b.s || (s == b.s && v < b.v)) { b.s = s; b.v = v; }
+}
+// Block-wide argmax (lowest index on ties); result valid in thread 0.
+__device__ __forceinline__ BestSV block_argmax(BestSV b, float* red_s, int* red_v) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const float os = __shfl_xor_sync(0xffffffffu, b.s, off);
+        const int ov = __shfl_xor_sync(0xffffffffu, b.v, off);
+        best_update(b, os, ov);
+    }
+    const int tid = threadIdx.x;
+    if ((tid & 31) == 0) { red_s[tid >> 5] = b.s; red_v[tid >> 5] = b.v; }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int wi = 1; wi < kFinWarps; ++wi) best_update(b, red_s[wi], red_v[wi]);
+    }
+    return b;
+}
+
+// Exact k-th largest (1-based, with multiplicity) of n keys in shared memory, by ONE warp:
+// MSB-first radix select, 8 bits per pass.  Requires 1 <= k <= n.
+struct SmemKeys {
+    const uint32_t* keys;
+    __device__ __forceinline__ uint32_t operator()(int e) const { return keys[e]; }
+};
+template <class Load>
+__device__ __forceinline__ uint32_t warp_radix_select(const Load load, int n, int k, int* hist, int lane) {
+    uint32_t prefix = 0u, mask = 0u;
+    for (int shift = 24; shift >= 0; shift -= 8) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) hist[lane * 8 + j] = 0;
+        __syncwarp();
+        for (int e = lane; e < n; e += 32) {
+            const uint32_t key = load(e);
+            if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1);
+        }
+        __syncwarp();
+        int cnt[8];
+        int sum = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { cnt[j] = hist[lane * 8 + j]; sum += cnt[j]; }
+        int incl = sum;  // inclusive suffix sum over lanes (higher lanes hold higher digits)
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int t = __shfl_down_sync(0xffffffffu, incl, off);
+            if (lane + off < 32) incl += t;
+        }
+        const int above = incl - sum;
+        uint32_t digit = 0;
+        int k_next = 0;
+        const bool mine = above < k && k <= above + sum;
+        if (mine) {
+            int a = above;
+#pragma unroll
+            for (int j = 7; j >= 0; --j) {
+                if (a < k && k <= a + cnt[j]) { digit = static_cast<uint32_t>(lane * 8 + j); k_next = k - a; break; }
+                a += cnt[j];
+            }
+        }
+        const uint32_t owner = __ballot_sync(0xffffffffu, mine);
+        const int src = __ffs(owner) - 1;
+        digit = __shfl_sync(0xffffffffu, digit, src);
+        k = __shfl_sync(0xffffffffu, k_next, src);
+        prefix |= digit << shift;
+        mask |= 0xffu << shift;
+        __syncwarp();
+    }
+    return prefix;
+}
+
+// EPT = keys per thread held in registers; supports V <= 256 * EPT.
+template <int EPT>
 __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const FinalizeParams p) {
-    extern __shared__ uint32_t keys[];  // [V]
+    extern __shared__ uint32_t dyn[];  // cand_key[V] | cand_idx[V]
     __shared__ int hist[256];
-    __shared__ uint32_t sel_prefix;
-    __shared__ int sel_k;
-    __shared__ float red_s[kFinThreads / 32];
-    __shared__ int red_v[kFinThreads / 32];
+    __shared__ uint32_t warp_kth[kFinWarps];
+    __shared__ int n_cand;
+    __shared__ uint32_t thr_key_s;
+    __shared__ float red_s[kFinWarps];
+    __shared__ int red_v[kFinWarps];
 
     const int i = blockIdx.x;   // stream
     const int r = blockIdx.y;   // batch row
     const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int warp = tid >> 5;
     const int pm = p.pair_map[r];
     if (pm >= 0 && (r & 1)) return;  // companion row: its cond row writes both
 
@@ -85,97 +182,306 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
 
     if (active) {
         const int V = p.V;
+        uint32_t* cand_key = dyn;
+        int* cand_idx = reinterpret_cast<int*>(dyn + V);
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
-        for (int v = tid; v < V; v += kFinThreads) keys[v] = float_key(zr[v]);
-        __syncthreads();
-
+        uint32_t key[EPT];
+#pragma unroll
+        for (int j = 0; j < EPT; ++j) {
+            const int v = j * kFinThreads + tid;
+            key[j] = v < V ? float_key(__ldg(zr + v)) : 0u;
+        }
         const float temp = p.temp[r];
         const int tk = p.top_k[r];
         const bool greedy = (tk == 1) || (temp == 0.f);
-        uint32_t thr_key = 0u;
-        if (!greedy && tk > 0 && tk < V) {
-            // exact k-th largest key: MSB-first radix select, 8 bits per pass
-            uint32_t prefix = 0u, mask = 0u;
-            int k_rem = tk;
-            for (int shift = 24; shift >= 0; shift -= 8) {
-                hist[tid] = 0;   // kFinThreads == 256 bins
-                __syncthreads();
-                for (int v = tid; v < V; v += kFinThreads) {
-                    const uint32_t key = keys[v];
-                    if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1);
-                }
-                __syncthreads();
-                if (tid < 32) {
-                    // lane l owns digits [8l, 8l+8); suffix sums over higher digits
-                    int cnt[8];
-                    int sum = 0;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) { cnt[j] = hist[tid * 8 + j]; sum += cnt[j]; }
-                    int above = 0;  // elements in lanes with higher digits
-                    int incl = sum;
-#pragma unroll
-                    for (int off = 1; off < 32; off <<= 1) {
-                        const int t = __shfl_down_sync(0xffffffffu, incl, off);
-                        if (tid + off < 32) incl += t;
-                    }
-                    above = incl - sum;
-                    // the k-th largest lies in this lane's digit range iff above < k_rem <= above + sum
-                    if (above < k_rem && k_rem <= above + sum) {
-                        int a = above;
-#pragma unroll
-                        for (int j = 7; j >= 0; --j) {
-                            if (a < k_rem && k_rem <= a + cnt[j]) {
-                                sel_prefix = prefix | (static_cast<uint32_t>(tid * 8 + j) << shift);
-                                sel_k = k_rem - a;
-                                break;
-                            }
-                            a += cnt[j];
-                        }
-                    }
-                }
-                __syncthreads();
-                prefix = sel_prefix;
-                k_rem = sel_k;
-                mask |= 0xffu << shift;
-                __syncthreads();
-            }
-            thr_key = prefix;
-        }
-
-        // argmax over survivors of s = z + g (or of z when greedy); lowest index wins ties
-        float best_s = -INFINITY;
-        int best_v = 0x7fffffff;
+        const bool filter = !greedy && tk > 0 && tk < V;
         const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
-        for (int v = tid; v < V; v += kFinThreads) {
-            const uint32_t key = keys[v];
-            if (key >= thr_key) {
-                float s = key_float(key);
-                if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v);
-                if (s > best_s || (s == best_s && v < best_v)) { best_s = s; best_v = v; }
-            }
-        }
+        BestSV best = {-INFINITY, 0x7fffffff};
+
+        if (filter) {
+            if (tid == 0) n_cand = 0;
+            // 1. lower bound L of the k-th largest key
+            uint32_t m = 0u;
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const float os = __shfl_xor_sync(0xffffffffu, best_s, off);
-            const int ov = __shfl_xor_sync(0xffffffffu, best_v, off);
-            if (os > best_s || (os == best_s && ov < best_v)) { best_s = os; best_v = ov; }
-        }
-        if ((tid & 31) == 0) { red_s[tid >> 5] = best_s; red_v[tid >> 5] = best_v; }
-        __syncthreads();
-        if (tid == 0) {
-            for (int wi = 1; wi < kFinThreads / 32; ++wi) {
-                const float os = red_s[wi];
-                const int ov = red_v[wi];
-                if (os > best_s || (os == best_s && ov < best_v)) { best_s = os; best_v = ov; }
+            for (int j = 0; j < EPT; ++j) m = max(m, key[j]);
+            const int kp = (tk + kFinWarps - 1) / kFinWarps;
+            uint32_t kth = 0u;
+            if (kp <= 32) {
+                uint32_t cur = m;
+                for (int it = 0; it < kp; ++it) {
+                    kth = __reduce_max_sync(0xffffffffu, cur);
+                    const uint32_t who = __ballot_sync(0xffffffffu, cur == kth);
+                    if (lane == __ffs(who) - 1) cur = 0u;
+                }
             }
-            token = best_v;
+            if (lane == 0) warp_kth[warp] = kth;
+            __syncthreads();
+            uint32_t L = warp_kth[0];
+#pragma unroll
+            for (int wi = 1; wi < kFinWarps; ++wi) L = min(L, warp_kth[wi]);
+            if (L == 0u) L = 1u;  // every real key
+            // 2. compact candidates (key >= L)
+#pragma unroll
+            for (int j = 0; j < EPT; ++j) {
+                const bool pred = key[j] >= L;
+                const uint32_t b = __ballot_sync(0xffffffffu, pred);
+                if (b) {
+                    int base = 0;
+                    if (lane == 0) base = atomicAdd(&n_cand, __popc(b));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (pred) {
+                        const int pos = base + __popc(b & ((1u << lane) - 1u));
+                        cand_key[pos] = key[j];
+                        cand_idx[pos] = j * kFinThreads + tid;
+                    }
+                }
+            }
+            __syncthreads();
+            const int C = n_cand;
+            // 3. exact threshold among the candidates
+            if (warp == 0) {
+                const uint32_t t = warp_radix_select(SmemKeys{cand_key}, C, tk, hist, lane);
+                if (lane == 0) thr_key_s = t;
+            }
+            __syncthreads();
+            const uint32_t thr_key = thr_key_s;
+            // 4. Gumbel-max over the survivors
+            for (int e = tid; e < C; e += kFinThreads) {
+                const uint32_t ck = cand_key[e];
+                if (ck >= thr_key) {
+                    const int v = cand_idx[e];
+                    best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                }
+            }
+        } else {
+            // greedy argmax, or no top-k filter: every token competes
+#pragma unroll
+            for (int j = 0; j < EPT; ++j) {
+                const int v = j * kFinThreads + tid;
+                if (v < V) {
+                    float s = key_float(key[j]);
+                    if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v);
+                    best_update(best, s, v);
+                }
+            }
         }
+        best = block_argmax(best, red_s, red_v);
+        token = best.v;
     }
     if (tid == 0) {
         p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
         if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
         if (p.delayed) {
-            const int slot = tau % p.T_cap;
+            const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
+            p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
+        }
+    }
+}
+
+// Fallback for V > 256 * 32: keys in shared memory, radix select over all of them.
+__global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const FinalizeParams p) {
+    extern __shared__ uint32_t dyn[];  // keys[V]
+    __shared__ int hist[256];
+    __shared__ uint32_t thr_key_s;
+    __shared__ float red_s[kFinWarps];
+    __shared__ int red_v[kFinWarps];
+
+    const int i = blockIdx.x, r = blockIdx.y, tid = threadIdx.x;
+    const int pm = p.pair_map[r];
+    if (pm >= 0 && (r & 1)) return;
+    const int tau = p.step[r];
+    const bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    int token = p.pad_token;
+    if (active) {
+        const int V = p.V;
+        const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
+        for (int v = tid; v < V; v += kFinThreads) dyn[v] = float_key(__ldg(zr + v));
+        __syncthreads();
+        const float temp = p.temp[r];
+        const int tk = p.top_k[r];
+        const bool greedy = (tk == 1) || (temp == 0.f);
+        uint32_t thr_key = 0u;
+        if (!greedy && tk > 0 && tk < V) {
+            if (tid < 32) {
+                const uint32_t t = warp_radix_select(SmemKeys{dyn}, V, tk, hist, tid);
+                if (tid == 0) thr_key_s = t;
+            }
+            __syncthreads();
+            thr_key = thr_key_s;
+        }
+        const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
+        BestSV best = {-INFINITY, 0x7fffffff};
+        for (int v = tid; v < V; v += kFinThreads) {
+            const uint32_t k = dyn[v];
+            if (k >= thr_key) {
+                float s = key_float(k);
+                if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v);
+                best_update(best, s, v);
+            }
+        }
+        best = block_argmax(best, red_s, red_v);
+        token = best.v;
+    }
+    if (tid == 0) {
+        p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
+        if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
+        if (p.delayed) {
+            const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
+            p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Candidate path (V % 32 == 0, V <= 8192): ONE WARP per (request-owning row, stream) works on the
+// V/8 values K1's epilogue emitted (top-4 of every 32-token chunk) instead of all V logits.
+//   t_E = k-th largest emitted value  <=  true threshold (the emitted set is a subset);
+//   a chunk whose 4th emitted value is < t_E cannot hide anything >= t_E, so its emitted values
+//   >= t_E are all of its candidates; a chunk whose 4th value reaches t_E ("overflow", rare) is
+//   re-read in full from the z spill.  The candidate set {z >= t_E} is then complete and the
+//   exact threshold is its k-th largest (= t_E when no chunk overflowed).
+// k > V/8 or no filter: the warp scans the full row from the spill (exact, slow, rare).
+constexpr int kCandWarps = 4;
+
+struct GlobalKeys {
+    const float* z;
+    __device__ __forceinline__ uint32_t operator()(int e) const { return float_key(__ldg(z + e)); }
+};
+
+__device__ __forceinline__ BestSV warp_argmax(BestSV b) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const float os = __shfl_xor_sync(0xffffffffu, b.s, off);
+        const int ov = __shfl_xor_sync(0xffffffffu, b.v, off);
+        best_update(b, os, ov);
+    }
+    return b;
+}
+
+__global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(const FinalizeParams p) {
+    extern __shared__ uint32_t dyn[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int cell = blockIdx.x * kCandWarps + warp;
+    if (cell >= p.R * p.S) return;
+    const int r = cell / p.S;
+    const int i = cell - r * p.S;
+    const int pm = p.pair_map[r];
+    if (pm >= 0 && (r & 1)) return;  // companion row
+
+    const int V = p.V;
+    const int G = V >> 5;            // chunks of this cell
+    const int E = G * 4;             // emitted values
+    // per-warp shared memory: keys[E] | src[G] | hist[256] | list_key[E + 32] | list_v[E + 32]
+    uint32_t* keys = dyn + static_cast<size_t>(warp) * (3 * E + G + 256 + 64);
+    uint32_t* srcs = keys + E;
+    int* hist = reinterpret_cast<int*>(srcs + G);
+    uint32_t* list_key = reinterpret_cast<uint32_t*>(hist + 256);
+    int* list_v = reinterpret_cast<int*>(list_key + E + 32);
+
+    const int tau = p.step[r];
+    const bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    int token = p.pad_token;
+    if (active) {
+        const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
+        const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
+        const float temp = p.temp[r];
+        const int tk = p.top_k[r];
+        const bool greedy = (tk == 1) || (temp == 0.f);
+        const bool filter = !greedy && tk > 0 && tk < V;
+        const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
+        BestSV best = {-INFINITY, 0x7fffffff};
+
+        if (greedy || (filter && tk <= E)) {
+            for (int e = lane; e < E; e += 32) keys[e] = float_key(__ldg(p.cand_val + chunk0 * 4 + e));
+            for (int c = lane; c < G; c += 32) srcs[c] = __ldg(p.cand_src + chunk0 + c);
+            __syncwarp();
+        }
+        if (greedy) {
+            // argmax = best chunk maximum; inside a chunk the emitted maximum is its lowest-index one
+            for (int c = lane; c < G; c += 32) best_update(best, key_float(keys[4 * c]), c * 32 + static_cast<int>(srcs[c] & 31u));
+        } else if (filter && tk <= E) {
+            const uint32_t tE = warp_radix_select(SmemKeys{keys}, E, tk, hist, lane);
+            // candidate list {z >= t_E}
+            int n_list = 0;
+            uint32_t any_overflow = 0u;
+            for (int c0 = 0; c0 < G; c0 += 32) {
+                const int c = c0 + lane;
+                const bool ovf = c < G && keys[4 * c + 3] >= tE;
+                any_overflow |= __ballot_sync(0xffffffffu, ovf);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const bool pred = c < G && !ovf && keys[4 * c + j] >= tE;
+                    const uint32_t b = __ballot_sync(0xffffffffu, pred);
+                    if (pred) {
+                        const int pos = n_list + __popc(b & ((1u << lane) - 1u));
+                        list_key[pos] = keys[4 * c + j];
+                        list_v[pos] = c * 32 + static_cast<int>((srcs[c] >> (8 * j)) & 31u);
+                    }
+                    n_list += __popc(b);
+                }
+            }
+            uint32_t thr = tE;
+            if (any_overflow) {
+                // re-read overflowing chunks in full (one coalesced 128-byte row each)
+                for (int c0 = 0; c0 < G; c0 += 32) {
+                    const int c = c0 + lane;
+                    uint32_t ovf_mask = __ballot_sync(0xffffffffu, c < G && keys[4 * c + 3] >= tE);
+                    while (ovf_mask) {
+                        const int cc = c0 + __ffs(ovf_mask) - 1;
+                        ovf_mask &= ovf_mask - 1u;
+                        const uint32_t k32 = float_key(__ldg(zr + cc * 32 + lane));
+                        const bool pred = k32 >= tE;
+                        const uint32_t b = __ballot_sync(0xffffffffu, pred);
+                        // the list has room for E + 32 entries; beyond that fall back to the full scan
+                        if (n_list + __popc(b) > E + 32) { n_list = -1; ovf_mask = 0u; c0 = G; break; }
+                        if (pred) {
+                            const int pos = n_list + __popc(b & ((1u << lane) - 1u));
+                            list_key[pos] = k32;
+                            list_v[pos] = cc * 32 + lane;
+                        }
+                        n_list += __popc(b);
+                    }
+                }
+                __syncwarp();
+                if (n_list >= 0) thr = warp_radix_select(SmemKeys{list_key}, n_list, tk, hist, lane);
+            }
+            __syncwarp();
+            if (n_list >= 0) {
+                for (int e = lane; e < n_list; e += 32) {
+                    const uint32_t ck = list_key[e];
+                    if (ck >= thr) {
+                        const int v = list_v[e];
+                        best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                    }
+                }
+            } else {
+                const uint32_t thr_full = warp_radix_select(GlobalKeys{zr}, V, tk, hist, lane);
+                for (int v = lane; v < V; v += 32) {
+                    const float zv = __ldg(zr + v);
+                    if (float_key(zv) >= thr_full)
+                        best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                }
+            }
+        } else {
+            // no top-k filter, or k larger than the emitted set: scan the whole row from the spill
+            uint32_t thr_full = 0u;
+            if (filter) thr_full = warp_radix_select(GlobalKeys{zr}, V, tk, hist, lane);
+            for (int v = lane; v < V; v += 32) {
+                const float zv = __ldg(zr + v);
+                if (float_key(zv) >= thr_full)
+                    best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+            }
+        }
+        best = warp_argmax(best);
+        token = best.v;
+    }
+    if (lane == 0) {
+        p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
+        if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
+        if (p.delayed) {
+            const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
             p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
         }
     }

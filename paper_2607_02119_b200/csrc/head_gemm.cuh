@@ -45,6 +45,8 @@ struct GemmParams {
     const float* bias;   // [NT]
     float* z;            // [R][NT]
     float* tap;          // nullable [R][NT]
+    float* cand_val;     // nullable [R][NT/32][4]: top-4 z of every 32-token chunk, descending
+    uint32_t* cand_src;  // nullable [R][NT/32]: their lane offsets inside the chunk, 8 bits each
     int* err;            // sticky error word {code | row << 8}
     uint64_t policy_w, policy_h;
 };
@@ -54,13 +56,30 @@ struct GemmSmemLayout {
     __host__ __device__ static constexpr uint32_t a_bytes() { return kBM * kBK * 2; }
     __host__ __device__ static constexpr uint32_t b_bytes(int BN) { return static_cast<uint32_t>(BN) * kBK * 2; }
     __host__ __device__ static constexpr uint32_t coef_bytes() { return (kMaxBN / 2) * sizeof(SlotCoef); }
-    __host__ __device__ static constexpr uint32_t misc_bytes() { return coef_bytes() + 256; }
+    __host__ __device__ static constexpr uint32_t stage_bytes() { return 32 * (kBM + 1) * 4; }  // candidate transpose
+    __host__ __device__ static constexpr uint32_t misc_bytes() { return coef_bytes() + 256 + stage_bytes(); }
     __host__ __device__ static constexpr uint32_t total(int BN, int stages) {
         return 1024 + stages * (a_bytes() + b_bytes(BN)) + misc_bytes();
     }
 };
 
-template <bool kTap>
+// Per-chunk candidate pass (north_star step 3, "per-N-tile top-k candidate pass held in
+// registers").  In this orientation a thread owns ONE token and many requests, the wrong axis
+// for a per-request top-k, so every 32-column accumulator slab is transposed through a 16 KB
+// shared-memory stage: afterwards epilogue thread (o, q) owns output column o (one request)
+// and the 32 tokens of vocabulary chunk q of the tile, and keeps the chunk's four largest z
+// (descending, lowest token first among equals) in registers with plain compares/selects.
+constexpr int kStageCols = 32;                 // output columns staged per round
+constexpr int kStagePitch = kBM + 1;           // words; +1 keeps both access patterns conflict-free
+__device__ __forceinline__ void top4_insert(float x, int e, float (&t)[4], int (&ix)[4]) {
+    const bool c0 = x > t[0], c1 = x > t[1], c2 = x > t[2], c3 = x > t[3];
+    t[3] = c2 ? t[2] : (c3 ? x : t[3]);   ix[3] = c2 ? ix[2] : (c3 ? e : ix[3]);
+    t[2] = c1 ? t[1] : (c2 ? x : t[2]);   ix[2] = c1 ? ix[1] : (c2 ? e : ix[2]);
+    t[1] = c0 ? t[0] : (c1 ? x : t[1]);   ix[1] = c0 ? ix[0] : (c1 ? e : ix[1]);
+    t[0] = c0 ? x : t[0];                 ix[0] = c0 ? e : ix[0];
+}
+
+template <bool kTap, bool kCand>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
                        const GemmParams p) {
@@ -79,9 +98,11 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
     const uint32_t bar_tfull = bar_base + 16 * kMaxStages;
     const uint32_t bar_tempty = bar_tfull + 16;
     const uint32_t tmem_ptr_smem = bar_tempty + 16;
+    const uint32_t smem_stage = bar_base + 256;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
     SlotCoef* coef = reinterpret_cast<SlotCoef*>(smem_gen + (smem_coef - smem_base));
     volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + (tmem_ptr_smem - smem_base));
+    float* stage = reinterpret_cast<float*>(smem_gen + (smem_stage - smem_base));
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -232,12 +253,33 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
                         const float z0 = fmaf(sc.c00, a0, fmaf(sc.c01, a1, bias * sc.d0));
                         p.z[static_cast<size_t>(r0) * p.NT + n] = z0;
                         if (kTap) p.tap[static_cast<size_t>(r0) * p.NT + n] = fmaf(sc.m00, a0, fmaf(sc.m01, a1, bias));
+                        if (kCand) stage[(2 * j) * kStagePitch + quarter * 32 + lane] = z0 + 0.0f;
                     }
                     if (n_ok && (kind & 2)) {
                         const float z1 = fmaf(sc.c11, a1, bias * sc.d1);
                         p.z[static_cast<size_t>(r0 + 1) * p.NT + n] = z1;
                         if (kTap) p.tap[static_cast<size_t>(r0 + 1) * p.NT + n] = a1 + bias;
+                        if (kCand) stage[(2 * j + 1) * kStagePitch + quarter * 32 + lane] = z1 + 0.0f;
                     }
+                }
+                if (kCand) {
+                    named_bar_sync(2, 128);                 // slab staged by all four epilogue warps
+                    const int o = et & 31;                  // output column of the slab
+                    const int q = et >> 5;                  // vocabulary chunk of the tile
+                    const int kind_o = coef[c * 16 + (o >> 1)].kind;
+                    const int nb = vt * kBM + q * 32;       // first token of the chunk (NT % 32 == 0)
+                    if (((kind_o >> (o & 1)) & 1) && nb < p.NT) {
+                        float t[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+                        int ix[4] = {0, 0, 0, 0};
+                        const float* col = stage + o * kStagePitch + q * 32;
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) top4_insert(col[e], e, t, ix);
+                        const size_t chunk = (static_cast<size_t>(row_base + o) * p.NT + nb) >> 5;
+                        *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(t[0], t[1], t[2], t[3]);
+                        p.cand_src[chunk] = static_cast<uint32_t>(ix[0]) | (static_cast<uint32_t>(ix[1]) << 8) |
+                                            (static_cast<uint32_t>(ix[2]) << 16) | (static_cast<uint32_t>(ix[3]) << 24);
+                    }
+                    named_bar_sync(2, 128);                 // stage may be overwritten
                 }
             }
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }

@@ -127,6 +127,10 @@ def _custom(pairs, singles, d, S, V, T=16, mixed=False, **kw):
     dict(pairs=20, singles=8, d=128, S=4, V=12800),       # 400 vocabulary tiles: >2 tiles per CTA
     dict(pairs=100, singles=0, d=512, S=2, V=640),        # R = 200 -> one 224-row tile
     dict(pairs=150, singles=0, d=256, S=2, V=384),        # R = 300 -> two row blocks
+    dict(pairs=3, singles=2, d=64, S=2, V=5000, top_k=700),    # 32 keys per thread; k > 256: no pruning bound
+    dict(pairs=2, singles=2, d=64, S=1, V=9000, top_k=40),     # V > 8192: shared-memory sampler fallback
+    dict(pairs=4, singles=0, d=64, S=2, V=1024, top_k=300),    # k > 256 with 4 keys per thread
+    dict(pairs=4, singles=0, d=64, S=2, V=300, top_k=299),     # k = V - 1
 ])
 def test_edge_shapes_full_oracle(dev, case):
     wl = _custom(**case)
@@ -135,6 +139,42 @@ def test_edge_shapes_full_oracle(dev, case):
     for t in (0, 1, wl.S, wl.T - 1):
         compare_step(dw, t, None, stats)
     print(case, stats.summary())
+
+
+def test_candidate_overflow_chunks_and_full_scan_agree(dev):
+    """The fused per-chunk top-4 candidate pass must stay exact when one 32-token chunk holds far more
+    than four of the top-k (it is re-read in full), and must give the tokens of the full-scan sampler."""
+    wl = _custom(pairs=6, singles=2, d=128, S=2, V=1024, top_k=40)
+    wl.heads[0, 64:90] *= 5.0           # 26 hot tokens inside chunk 2 of stream 0 (and chunk 2 only partly)
+    wl.heads[1, 500:520] *= 4.0         # straddles chunks 15 and 16 of stream 1
+    stats = ParityStats()
+    dw = DeviceWorkload(wl, dev)
+    for t in (3, 8, 12):
+        compare_step(dw, t, None, stats)
+    print("overflow:", stats.summary())
+    full = DeviceWorkload(wl, dev, no_candidates=True)
+    for t in (3, 8):
+        dw.step(t)
+        full.step(t)
+        torch.cuda.synchronize()
+        assert torch.equal(dw.tokens, full.tokens)
+    # the full-scan sampler on its own is also exact against the oracle
+    s2 = ParityStats()
+    compare_step(full, 5, None, s2)
+    # every per-row mode of the candidate path against the full-scan path at a BASELINE shape
+    wl2 = _custom(pairs=24, singles=16, d=256, S=4, V=2048, mixed=True)
+    heads = wl2.head_rows()
+    modes = [0, 1, 20, 50, 256, 257, 2047, 2048, 5000, -1]
+    for q, r in enumerate(heads):
+        wl2.top_k[r] = modes[q % len(modes)]
+    a, b = DeviceWorkload(wl2, dev), DeviceWorkload(wl2, dev, no_candidates=True)
+    s3 = ParityStats()
+    compare_step(a, 9, None, s3)
+    for t in (4, 9):
+        a.step(t)
+        b.step(t)
+        torch.cuda.synchronize()
+        assert torch.equal(a.tokens, b.tokens)
 
 
 def test_row_tile_override_many_row_blocks(dev):
