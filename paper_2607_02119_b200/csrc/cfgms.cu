@@ -86,11 +86,21 @@ void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb) {
         *nrb = (R + *BN - 1) / *BN;
         return;
     }
-    int blocks = (R + kMaxBN - 1) / kMaxBN;
-    int per = (R + blocks - 1) / blocks;
-    per = ((per + 31) / 32) * 32;
-    *BN = per;
-    *nrb = (R + per - 1) / per;
+    // Cost model: a CTA's time for one tile is ~ the bytes it pulls per K step, (128 + BN) rows of
+    // 128 B, and the slowest CTA runs ceil(tiles / SMs) tiles.  Splitting the rows re-reads the
+    // weight tile from L2 (not HBM) but lets small batches occupy every SM.
+    const int vt = (c->NT + kBM - 1) / kBM;
+    const int min_blocks = (R + kMaxBN - 1) / kMaxBN;
+    long best_cost = -1;
+    for (int blocks = min_blocks; blocks <= min_blocks * 8; ++blocks) {
+        int per = (R + blocks - 1) / blocks;
+        per = ((per + 31) / 32) * 32;
+        const int nb = (R + per - 1) / per;
+        const long waves = (static_cast<long>(vt) * nb + c->num_sms - 1) / c->num_sms;
+        const long cost = waves * (kBM + per + 16);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; *BN = per; *nrb = nb; }
+        if (per <= 32) break;
+    }
 }
 
 template <typename T>
@@ -208,7 +218,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
                              c->max_smem_optin) != cudaSuccess ||
         cudaFuncSetAttribute(cfgms_head_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              c->max_smem_optin) != cudaSuccess ||
-        cudaFuncSetAttribute(cfgms_finalize_cand_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(cfgms_finalize_cand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
         max_gemm_smem > c->max_smem_optin) {
         cfgms_destroy(c);
         return CFGMS_ERR_CUDA;
@@ -313,10 +323,13 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
     fp.cand_val = c->cand_val; fp.cand_src = c->cand_src;
     if (c->use_cand) {
-        const int G = c->V / 32, E = 4 * G;
-        const size_t fsmem = static_cast<size_t>(kCandWarps) * (3 * E + G + 256 + 64) * 4;
+        const size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;
         const int cells = a->R * c->S;
-        cfgms_finalize_cand_kernel<<<(cells + kCandWarps - 1) / kCandWarps, kCandWarps * 32, fsmem, st>>>(fp);
+        const int fblocks = (cells + kCandWarps - 1) / kCandWarps;
+        if (c->V <= 1024) cfgms_finalize_cand_kernel<1><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
+        else if (c->V <= 2048) cfgms_finalize_cand_kernel<2><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
+        else if (c->V <= 4096) cfgms_finalize_cand_kernel<4><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
+        else cfgms_finalize_cand_kernel<8><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
     } else {
         const dim3 fgrid(c->S, a->R);
         const size_t fsmem = static_cast<size_t>(c->V) * 8;

@@ -81,6 +81,12 @@ __device__ __forceinline__ float key_float(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
 
+// Key of a value that is already canonical (K1 stores z + 0.0f) and not NaN: two instructions.
+__device__ __forceinline__ uint32_t float_key_fast(float f) {
+    const uint32_t u = __float_as_uint(f);
+    return u ^ (static_cast<uint32_t>(static_cast<int32_t>(u) >> 31) | 0x80000000u);
+}
+
 struct BestSV {
     float s;
     int v;
@@ -335,12 +341,16 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
 
 // ---------------------------------------------------------------------------------------------
 // Candidate path (V % 32 == 0, V <= 8192): ONE WARP per (request-owning row, stream) works on the
-// V/8 values K1's epilogue emitted (top-4 of every 32-token chunk) instead of all V logits.
+// V/8 values K1's epilogue emitted (top-4 of every 32-token chunk, descending) instead of all V
+// logits.  Lane l keeps chunks l, l+32, ... in registers.
 //   t_E = k-th largest emitted value  <=  true threshold (the emitted set is a subset);
 //   a chunk whose 4th emitted value is < t_E cannot hide anything >= t_E, so its emitted values
 //   >= t_E are all of its candidates; a chunk whose 4th value reaches t_E ("overflow", rare) is
 //   re-read in full from the z spill.  The candidate set {z >= t_E} is then complete and the
 //   exact threshold is its k-th largest (= t_E when no chunk overflowed).
+// t_E itself: with j = ceil(k / G), lo = min over chunks of their j-th value is a lower bound
+// (G*j >= k values are >= lo); ONE histogram pass with 256 linear buckets over [lo, max] finds
+// the bucket of the k-th largest, and the few values of that bucket are ranked exactly.
 // k > V/8 or no filter: the warp scans the full row from the spill (exact, slow, rare).
 constexpr int kCandWarps = 4;
 
@@ -359,6 +369,11 @@ __device__ __forceinline__ BestSV warp_argmax(BestSV b) {
     return b;
 }
 
+// per-warp shared memory (32-bit words): hist[256] | small[32] | misc[8] | list_key[cap] | list_v[cap]
+__host__ __device__ constexpr int cand_list_cap(int V) { return V / 8 + 32; }
+__host__ __device__ constexpr int cand_warp_words(int V) { return 256 + 32 + 8 + 2 * cand_list_cap(V); }
+
+template <int CPL>   // chunks per lane: V <= 1024 * CPL
 __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(const FinalizeParams p) {
     extern __shared__ uint32_t dyn[];
     const int lane = threadIdx.x & 31;
@@ -373,12 +388,12 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     const int V = p.V;
     const int G = V >> 5;            // chunks of this cell
     const int E = G * 4;             // emitted values
-    // per-warp shared memory: keys[E] | src[G] | hist[256] | list_key[E + 32] | list_v[E + 32]
-    uint32_t* keys = dyn + static_cast<size_t>(warp) * (3 * E + G + 256 + 64);
-    uint32_t* srcs = keys + E;
-    int* hist = reinterpret_cast<int*>(srcs + G);
-    uint32_t* list_key = reinterpret_cast<uint32_t*>(hist + 256);
-    int* list_v = reinterpret_cast<int*>(list_key + E + 32);
+    const int cap = cand_list_cap(V);
+    int* hist = reinterpret_cast<int*>(dyn + static_cast<size_t>(warp) * cand_warp_words(V));
+    uint32_t* small = reinterpret_cast<uint32_t*>(hist + 256);
+    int* misc = reinterpret_cast<int*>(small + 32);
+    uint32_t* list_key = reinterpret_cast<uint32_t*>(misc + 8);
+    int* list_v = reinterpret_cast<int*>(list_key + cap);
 
     const int tau = p.step[r];
     const bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
@@ -394,74 +409,194 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         BestSV best = {-INFINITY, 0x7fffffff};
 
         if (greedy || (filter && tk <= E)) {
-            for (int e = lane; e < E; e += 32) keys[e] = float_key(__ldg(p.cand_val + chunk0 * 4 + e));
-            for (int c = lane; c < G; c += 32) srcs[c] = __ldg(p.cand_src + chunk0 + c);
-            __syncwarp();
-        }
-        if (greedy) {
-            // argmax = best chunk maximum; inside a chunk the emitted maximum is its lowest-index one
-            for (int c = lane; c < G; c += 32) best_update(best, key_float(keys[4 * c]), c * 32 + static_cast<int>(srcs[c] & 31u));
-        } else if (filter && tk <= E) {
-            const uint32_t tE = warp_radix_select(SmemKeys{keys}, E, tk, hist, lane);
-            // candidate list {z >= t_E}
-            int n_list = 0;
-            uint32_t any_overflow = 0u;
-            for (int c0 = 0; c0 < G; c0 += 32) {
-                const int c = c0 + lane;
-                const bool ovf = c < G && keys[4 * c + 3] >= tE;
-                any_overflow |= __ballot_sync(0xffffffffu, ovf);
+            uint32_t key[CPL][4];
+            uint32_t src[CPL];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const bool pred = c < G && !ovf && keys[4 * c + j] >= tE;
-                    const uint32_t b = __ballot_sync(0xffffffffu, pred);
-                    if (pred) {
-                        const int pos = n_list + __popc(b & ((1u << lane) - 1u));
-                        list_key[pos] = keys[4 * c + j];
-                        list_v[pos] = c * 32 + static_cast<int>((srcs[c] >> (8 * j)) & 31u);
-                    }
-                    n_list += __popc(b);
+            for (int j = 0; j < CPL; ++j) {
+                const int c = j * 32 + lane;
+                if (c < G) {
+                    const float4 v4 = __ldg(reinterpret_cast<const float4*>(p.cand_val) + chunk0 + c);
+                    src[j] = __ldg(p.cand_src + chunk0 + c);
+                    key[j][0] = float_key_fast(v4.x); key[j][1] = float_key_fast(v4.y);
+                    key[j][2] = float_key_fast(v4.z); key[j][3] = float_key_fast(v4.w);
+                } else {
+                    src[j] = 0u;
+                    key[j][0] = key[j][1] = key[j][2] = key[j][3] = 0u;
                 }
             }
-            uint32_t thr = tE;
-            if (any_overflow) {
-                // re-read overflowing chunks in full (one coalesced 128-byte row each)
-                for (int c0 = 0; c0 < G; c0 += 32) {
-                    const int c = c0 + lane;
-                    uint32_t ovf_mask = __ballot_sync(0xffffffffu, c < G && keys[4 * c + 3] >= tE);
-                    while (ovf_mask) {
-                        const int cc = c0 + __ffs(ovf_mask) - 1;
-                        ovf_mask &= ovf_mask - 1u;
-                        const uint32_t k32 = float_key(__ldg(zr + cc * 32 + lane));
-                        const bool pred = k32 >= tE;
+            if (greedy) {
+                // argmax = best chunk maximum; inside a chunk the emitted maximum is its lowest-index one
+#pragma unroll
+                for (int j = 0; j < CPL; ++j)
+                    if (j * 32 + lane < G)
+                        best_update(best, key_float(key[j][0]), (j * 32 + lane) * 32 + static_cast<int>(src[j] & 31u));
+            } else {
+                // ---- t_E: k-th largest of the E emitted values
+                const int jj = (tk + G - 1) / G - 1;           // 0..3: the (jj+1)-th value of every chunk
+                uint32_t lo = 0xffffffffu, hi = 0u;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) {
+                    if (j * 32 + lane < G) {
+                        const uint32_t kj = jj == 0 ? key[j][0] : jj == 1 ? key[j][1] : jj == 2 ? key[j][2] : key[j][3];
+                        lo = min(lo, kj);
+                        hi = max(hi, key[j][0]);
+                    }
+                }
+                lo = __reduce_min_sync(0xffffffffu, lo);
+                hi = __reduce_max_sync(0xffffffffu, hi);
+                const uint32_t range = hi - lo;
+                const int shift = range < 256u ? 0 : (24 - __clz(range));   // (key - lo) >> shift <= 255
+#pragma unroll
+                for (int j = 0; j < 8; ++j) hist[lane * 8 + j] = 0;
+                if (lane == 0) misc[0] = 0;
+                __syncwarp();
+#pragma unroll
+                for (int j = 0; j < CPL; ++j)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e)
+                        if (key[j][e] >= lo) atomicAdd(&hist[(key[j][e] - lo) >> shift], 1);
+                __syncwarp();
+                int cnt[8];
+                int sum = 0;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) { cnt[j] = hist[lane * 8 + j]; sum += cnt[j]; }
+                int incl = sum;
+#pragma unroll
+                for (int off = 1; off < 32; off <<= 1) {
+                    const int t = __shfl_down_sync(0xffffffffu, incl, off);
+                    if (lane + off < 32) incl += t;
+                }
+                const int above = incl - sum;
+                int bucket = 0, k_rem = 0, m_in = 0;
+                const bool mine = above < tk && tk <= above + sum;
+                if (mine) {
+                    int a = above;
+#pragma unroll
+                    for (int j = 7; j >= 0; --j) {
+                        if (a < tk && tk <= a + cnt[j]) { bucket = lane * 8 + j; k_rem = tk - a; m_in = cnt[j]; break; }
+                        a += cnt[j];
+                    }
+                }
+                const int owner = __ffs(__ballot_sync(0xffffffffu, mine)) - 1;
+                bucket = __shfl_sync(0xffffffffu, bucket, owner);
+                k_rem = __shfl_sync(0xffffffffu, k_rem, owner);
+                m_in = __shfl_sync(0xffffffffu, m_in, owner);
+                uint32_t tE = 0u;
+                if (m_in <= 32) {
+                    // rank the few values of that bucket exactly
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (key[j][e] >= lo && static_cast<int>((key[j][e] - lo) >> shift) == bucket)
+                                small[atomicAdd(&misc[0], 1)] = key[j][e];
+                    __syncwarp();
+                    const uint32_t x = lane < m_in ? small[lane] : 0u;
+                    int gt = 0, ge = 0;
+                    for (int q = 0; q < m_in; ++q) {
+                        const uint32_t y = small[q];
+                        gt += y > x;
+                        ge += y >= x;
+                    }
+                    const bool hit = lane < m_in && gt < k_rem && k_rem <= ge;
+                    const int who = __ffs(__ballot_sync(0xffffffffu, hit)) - 1;
+                    tE = __shfl_sync(0xffffffffu, x, who);
+                } else {
+                    // many (near-)equal values in one bucket: generic radix select over all emitted values
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (j * 32 + lane < G) list_key[(j * 32 + lane) * 4 + e < cap ? (j * 32 + lane) * 4 + e : 0] = key[j][e];
+                    __syncwarp();
+                    tE = E <= cap ? warp_radix_select(SmemKeys{list_key}, E, tk, hist, lane) : 0u;
+                    __syncwarp();
+                }
+                // ---- candidate list {z >= t_E}; overflowing chunks are re-read in full
+                int n_list = 0;
+                uint32_t any_overflow = 0u;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) {
+                    const int c = j * 32 + lane;
+                    const bool ovf = c < G && key[j][3] >= tE;
+                    any_overflow |= __ballot_sync(0xffffffffu, ovf);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const bool pred = c < G && !ovf && key[j][e] >= tE;
                         const uint32_t b = __ballot_sync(0xffffffffu, pred);
-                        // the list has room for E + 32 entries; beyond that fall back to the full scan
-                        if (n_list + __popc(b) > E + 32) { n_list = -1; ovf_mask = 0u; c0 = G; break; }
                         if (pred) {
                             const int pos = n_list + __popc(b & ((1u << lane) - 1u));
-                            list_key[pos] = k32;
-                            list_v[pos] = cc * 32 + lane;
+                            list_key[pos] = key[j][e];
+                            list_v[pos] = c * 32 + static_cast<int>((src[j] >> (8 * e)) & 31u);
                         }
                         n_list += __popc(b);
                     }
                 }
-                __syncwarp();
-                if (n_list >= 0) thr = warp_radix_select(SmemKeys{list_key}, n_list, tk, hist, lane);
-            }
-            __syncwarp();
-            if (n_list >= 0) {
-                for (int e = lane; e < n_list; e += 32) {
-                    const uint32_t ck = list_key[e];
-                    if (ck >= thr) {
-                        const int v = list_v[e];
-                        best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                uint32_t thr = tE;
+                if (any_overflow) {
+                    int n_new = 0;   // values >= t_E that were hidden behind a chunk's four emitted ones
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j) {
+                        uint32_t ovf_mask = __ballot_sync(0xffffffffu, j * 32 + lane < G && key[j][3] >= tE);
+                        while (ovf_mask && n_list >= 0) {
+                            const int cc = j * 32 + __ffs(ovf_mask) - 1;
+                            ovf_mask &= ovf_mask - 1u;
+                            const uint32_t k32 = float_key(__ldg(zr + cc * 32 + lane));
+                            const bool pred = k32 >= tE;
+                            const uint32_t b = __ballot_sync(0xffffffffu, pred);
+                            if (n_list + __popc(b) > cap) { n_list = -1; break; }   // too many ties: full scan
+                            if (pred) {
+                                const int pos = n_list + __popc(b & ((1u << lane) - 1u));
+                                list_key[pos] = k32;
+                                list_v[pos] = cc * 32 + lane;
+                            }
+                            n_list += __popc(b);
+                            n_new += __popc(b) - 4;
+                        }
+                    }
+                    __syncwarp();
+                    if (n_list >= 0 && n_new > 0) {
+                        // exact threshold of the completed set = its k-th largest: drop the (n_list - k) smallest
+                        const int extra = n_list - tk;
+                        if (extra <= 8) {
+                            for (int it = 0;; ++it) {
+                                uint32_t mine_min = 0xffffffffu;
+                                int mine_pos = 0;
+                                for (int e = lane; e < n_list; e += 32) {
+                                    const uint32_t ck = list_key[e];
+                                    if (list_v[e] >= 0 && ck < mine_min) { mine_min = ck; mine_pos = e; }
+                                }
+                                thr = __reduce_min_sync(0xffffffffu, mine_min);
+                                if (it == extra) break;
+                                const uint32_t holder = __ballot_sync(0xffffffffu, mine_min == thr);
+                                if (lane == __ffs(holder) - 1) list_v[mine_pos] = -1 - list_v[mine_pos];   // drop one instance
+                                __syncwarp();
+                            }
+                            // dropped entries are <= thr; those tying it still survive (threshold semantics)
+                            for (int e = lane; e < n_list; e += 32)
+                                if (list_v[e] < 0) list_v[e] = -1 - list_v[e];
+                            __syncwarp();
+                        } else {
+                            thr = warp_radix_select(SmemKeys{list_key}, n_list, tk, hist, lane);
+                        }
                     }
                 }
-            } else {
-                const uint32_t thr_full = warp_radix_select(GlobalKeys{zr}, V, tk, hist, lane);
-                for (int v = lane; v < V; v += 32) {
-                    const float zv = __ldg(zr + v);
-                    if (float_key(zv) >= thr_full)
-                        best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                __syncwarp();
+                if (n_list >= 0) {
+                    for (int e = lane; e < n_list; e += 32) {
+                        const uint32_t ck = list_key[e];
+                        if (ck >= thr) {
+                            const int v = list_v[e];
+                            best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                        }
+                    }
+                } else {
+                    const uint32_t thr_full = warp_radix_select(GlobalKeys{zr}, V, tk, hist, lane);
+                    for (int v = lane; v < V; v += 32) {
+                        const float zv = __ldg(zr + v);
+                        if (float_key(zv) >= thr_full)
+                            best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                    }
                 }
             }
         } else {
