@@ -96,6 +96,8 @@ class ClockSampler:
 class Runner:
     """One config resident on one GPU, stepping through the C ABI."""
 
+    cta_pair = None   # tuning override (--cta-pair): None = library default
+
     def __init__(self, cfg: int, dev, cfg_off: bool = False, rank: int = 0, n_ranks: int = 1):
         import torch
         import paper_2607_02119_b200 as pkg
@@ -111,7 +113,7 @@ class Runner:
         self.wl, self.dev = wl, dev
         cu = lambda t: None if t is None else t.to(dev)
         self.heads, self.embeds = cu(wl.heads), cu(wl.embeds)
-        self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2))
+        self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), cta_pair=Runner.cta_pair)
         self.pool = cu(wl.hidden_pool)
         self.pair_map, self.w, self.temp, self.top_k = cu(wl.pair_map), cu(wl.w), cu(wl.temp), cu(wl.top_k)
         self.req_id, self.n_frames = cu(wl.req_id), cu(wl.n_frames)
@@ -315,7 +317,10 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip ratio / other configs / cold-L2 legs")
+    ap.add_argument("--cta-pair", default="auto", choices=["auto", "on", "off"],
+                    help="tuning: force the CTA-pair (cta_group::2) or the one-CTA head GEMM")
     args = ap.parse_args()
+    Runner.cta_pair = {"auto": None, "on": True, "off": False}[args.cta_pair]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
@@ -366,7 +371,7 @@ def main():
                                    wl.heads.numel() * 2 / 2 ** 20, wl.hidden_pool.numel() * wl.hidden_pool.element_size() / 2 ** 20,
                                    wl.n_req * wl.S * wl.V * 4 / 2 ** 20),
                                row_tile=info["row_tile"], row_blocks=info["row_blocks"], gemm_grid=info["gemm_grid"],
-                               pipeline_stages=info["pipeline_stages"]),
+                               pipeline_stages=info["pipeline_stages"], cta_pair=bool(info["cta_pair"])),
                 "clocks": sampler.summary(), "gpu_launches": int(info["launches_last_step"] * K + 1), "roofline": roof}
 
     # end-to-end through the host-buffer entry point (every rank, max over ranks)

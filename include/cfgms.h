@@ -55,11 +55,14 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
                                       the sampler then scans all V logits of every cell (the path
                                       always taken when V % 32 != 0 or V > 8192)                 */
 
+#define CFGMS_CFG_SINGLE_CTA 4u  /* tuning/debug: never pair CTAs on one M = 256 MMA                */
+#define CFGMS_CFG_CTA_PAIR 8u    /* tuning/debug: always run the head GEMM on CTA pairs (cta_group::2) */
+
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
     int32_t pad_token; /* written at inactive (step, stream) cells when CFGMS_CFG_PAD_TOKEN      */
     uint32_t flags;
-    int32_t row_tile;  /* debug/tuning: batch rows per accumulator tile (multiple of 32,
+    int32_t row_tile;  /* debug/tuning: batch rows per accumulator tile (multiple of 64,
                           <= 256); 0 = chosen from R and the SM count                           */
     int32_t reserved[4];
 } cfgms_config;
@@ -155,6 +158,8 @@ typedef struct {
     int64_t launches_total;        /* kernels enqueued since create                             */
     int64_t h2d_bytes_last_step;   /* cfgms_step_host only                                      */
     int64_t d2h_bytes_last_step;
+    int32_t cta_pair;              /* 1 when the last head GEMM ran on CTA pairs (cta_group::2) */
+    int32_t reserved_;
 } cfgms_info;
 int cfgms_get_info(cfgms_ctx* ctx, cfgms_info* out);
 

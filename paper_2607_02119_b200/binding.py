@@ -15,6 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libcfgms.so")
 CFGMS_BF16, CFGMS_F32 = 0, 1
 CFGMS_CFG_PAD_TOKEN = 1
 CFGMS_CFG_NO_CANDIDATES = 2
+CFGMS_CFG_SINGLE_CTA = 4
+CFGMS_CFG_CTA_PAIR = 8
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
           5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
@@ -49,7 +51,7 @@ class cfgms_info(C.Structure):
                 ("row_blocks", C.c_int32), ("vocab_tiles", C.c_int32), ("gemm_grid", C.c_int32),
                 ("pipeline_stages", C.c_int32), ("launches_last_step", C.c_int32),
                 ("launches_total", C.c_int64), ("h2d_bytes_last_step", C.c_int64),
-                ("d2h_bytes_last_step", C.c_int64)]
+                ("d2h_bytes_last_step", C.c_int64), ("cta_pair", C.c_int32), ("reserved_", C.c_int32)]
 
 
 _LIB = None
@@ -127,7 +129,8 @@ class Context:
     """cfgms_create / cfgms_destroy.  `heads` (bf16 [S][V][d], cuda) is borrowed: kept alive here."""
 
     def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
-                 pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False):
+                 pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
+                 cta_pair: Optional[bool] = None):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -142,6 +145,8 @@ class Context:
             cfg.flags |= CFGMS_CFG_PAD_TOKEN
         if no_candidates:
             cfg.flags |= CFGMS_CFG_NO_CANDIDATES
+        if cta_pair is not None:   # tuning: force the one-CTA or the CTA-pair head GEMM
+            cfg.flags |= CFGMS_CFG_CTA_PAIR if cta_pair else CFGMS_CFG_SINGLE_CTA
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):

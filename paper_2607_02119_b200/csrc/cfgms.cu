@@ -41,6 +41,7 @@ struct cfgms_ctx {
     int S = 0, d = 0, V = 0, NT = 0;
     int device = 0, num_sms = 0;
     int max_rows = 0, pad_token = 0, row_tile_override = 0;
+    int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT]
     float* z = nullptr;               // [max_rows][NT]
@@ -53,7 +54,7 @@ struct cfgms_ctx {
     CUtensorMap tmap_w;
     CUtensorMap tmap_h;
     const void* tmap_h_ptr = nullptr;
-    int tmap_h_R = 0, tmap_h_BN = 0;
+    int tmap_h_R = 0, tmap_h_box = 0;
     int max_smem_optin = 0;
     HostStage hs;
     bool hs_ready = false;
@@ -77,30 +78,33 @@ int make_tmap_2d(cfgms_ctx* c, CUtensorMap* m, const void* base, uint64_t rows, 
     return r == CUDA_SUCCESS ? CFGMS_OK : CFGMS_ERR_CUDA;
 }
 
-// Batch rows per accumulator tile: as few row blocks as TMEM allows (N <= 256 per MMA, two
-// accumulator stages in 512 columns), each a multiple of 32 columns so that a pair never
-// straddles a tile and tcgen05.ld.x32 chunks are whole.
-void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb) {
+// Batch rows per accumulator tile (BN, a multiple of 64 = one slab pair of the epilogue, <= 256 =
+// UMMA N with two accumulator stages in 512 TMEM columns) and whether two CTAs pair up on one
+// M = 256 MMA.  A (cond, uncond) pair never straddles a tile because BN is even.
+void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb, bool* pair) {
+    const int vt = (c->NT + kBM - 1) / kBM;
     if (c->row_tile_override > 0) {
         *BN = c->row_tile_override;
         *nrb = (R + *BN - 1) / *BN;
-        return;
+    } else {
+        // Cost model: a CTA's time for one tile is ~ the bytes it pulls per K step, (128 + BN) rows of
+        // 128 B, and the slowest CTA runs ceil(tiles / SMs) tiles.  Splitting the rows re-reads the
+        // weight tile from L2 (not HBM) but lets small batches occupy every SM.
+        const int min_blocks = (R + kMaxBN - 1) / kMaxBN;
+        long best_cost = -1;
+        for (int blocks = min_blocks; blocks <= min_blocks * 8; ++blocks) {
+            int per = (R + blocks - 1) / blocks;
+            per = ((per + 63) / 64) * 64;
+            const int nb = (R + per - 1) / per;
+            const long waves = (static_cast<long>(vt) * nb + c->num_sms - 1) / c->num_sms;
+            const long cost = waves * (kBM + per + 16);
+            if (best_cost < 0 || cost < best_cost) { best_cost = cost; *BN = per; *nrb = nb; }
+            if (per <= 64) break;
+        }
     }
-    // Cost model: a CTA's time for one tile is ~ the bytes it pulls per K step, (128 + BN) rows of
-    // 128 B, and the slowest CTA runs ceil(tiles / SMs) tiles.  Splitting the rows re-reads the
-    // weight tile from L2 (not HBM) but lets small batches occupy every SM.
-    const int vt = (c->NT + kBM - 1) / kBM;
-    const int min_blocks = (R + kMaxBN - 1) / kMaxBN;
-    long best_cost = -1;
-    for (int blocks = min_blocks; blocks <= min_blocks * 8; ++blocks) {
-        int per = (R + blocks - 1) / blocks;
-        per = ((per + 31) / 32) * 32;
-        const int nb = (R + per - 1) / per;
-        const long waves = (static_cast<long>(vt) * nb + c->num_sms - 1) / c->num_sms;
-        const long cost = waves * (kBM + per + 16);
-        if (best_cost < 0 || cost < best_cost) { best_cost = cost; *BN = per; *nrb = nb; }
-        if (per <= 32) break;
-    }
+    // Pairing halves the row-operand traffic per SM; it pays once the row tile is large (the
+    // tensor-bound regime).  Small batches stream weights and want as many independent CTAs as possible.
+    *pair = c->pair_mode == 2 || (c->pair_mode == 0 && *BN >= 128 && vt >= 2);
 }
 
 template <typename T>
@@ -162,7 +166,8 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     c->max_rows = (cfg && cfg->max_rows > 0) ? cfg->max_rows : 1024;
     c->pad_token = (cfg && (cfg->flags & CFGMS_CFG_PAD_TOKEN)) ? cfg->pad_token : V;
     c->row_tile_override = cfg ? cfg->row_tile : 0;
-    if (c->row_tile_override < 0 || c->row_tile_override > kMaxBN || (c->row_tile_override % 32) != 0) {
+    c->pair_mode = (cfg && (cfg->flags & CFGMS_CFG_SINGLE_CTA)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_CTA_PAIR)) ? 2 : 0;
+    if (c->row_tile_override < 0 || c->row_tile_override > kMaxBN || (c->row_tile_override % 64) != 0) {
         delete c;
         return CFGMS_ERR_ARG;
     }
@@ -209,17 +214,20 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
             return CFGMS_ERR_CUDA;
         }
     }
-    const int max_gemm_smem = static_cast<int>(GemmSmemLayout::total(kMaxBN, 4));
-    if (cudaFuncSetAttribute(cfgms_head_gemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             c->max_smem_optin) != cudaSuccess ||
-        cudaFuncSetAttribute(cfgms_head_gemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             c->max_smem_optin) != cudaSuccess ||
-        cudaFuncSetAttribute(cfgms_head_gemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             c->max_smem_optin) != cudaSuccess ||
-        cudaFuncSetAttribute(cfgms_head_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             c->max_smem_optin) != cudaSuccess ||
-        cudaFuncSetAttribute(cfgms_finalize_cand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
-        max_gemm_smem > c->max_smem_optin) {
+    bool attr_ok = static_cast<int>(GemmSmemLayout::total(kMaxBN, 2)) <= c->max_smem_optin;
+    auto set_smem = [&](const void* fn) {
+        attr_ok = attr_ok && cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin) == cudaSuccess;
+    };
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<false, false, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, false, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<false, true, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, true, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<false, false, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, false, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<false, true, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, true, true>));
+    if (!attr_ok ||
+        cudaFuncSetAttribute(cfgms_finalize_cand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
         cfgms_destroy(c);
         return CFGMS_ERR_CUDA;
     }
@@ -275,21 +283,23 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     if ((reinterpret_cast<uintptr_t>(hidden) & 15u) != 0) return CFGMS_ERR_ARG;
 
     int BN, nrb;
-    choose_row_tile(c, a->R, &BN, &nrb);
-    if (c->tmap_h_ptr != hidden || c->tmap_h_R != a->R || c->tmap_h_BN != BN) {
+    bool pair;
+    choose_row_tile(c, a->R, &BN, &nrb, &pair);
+    const int b_rows = pair ? BN / 2 : BN;     // batch rows one CTA stages per K block (TMA box height)
+    if (c->tmap_h_ptr != hidden || c->tmap_h_R != a->R || c->tmap_h_box != b_rows) {
         rc = make_tmap_2d(c, &c->tmap_h, hidden, static_cast<uint64_t>(a->R), static_cast<uint64_t>(c->d),
-                          static_cast<uint32_t>(BN));
+                          static_cast<uint32_t>(b_rows));
         if (rc != CFGMS_OK) return rc;
-        c->tmap_h_ptr = hidden; c->tmap_h_R = a->R; c->tmap_h_BN = BN;
+        c->tmap_h_ptr = hidden; c->tmap_h_R = a->R; c->tmap_h_box = b_rows;
     }
 
     GemmParams gp;
     gp.R = a->R; gp.NT = c->NT; gp.d = c->d; gp.BN = BN;
     gp.num_row_blocks = nrb;
     gp.num_vocab_tiles = (c->NT + kBM - 1) / kBM;
-    gp.num_tiles = gp.num_vocab_tiles * nrb;
+    gp.num_tiles = (pair ? (gp.num_vocab_tiles + 1) / 2 : gp.num_vocab_tiles) * nrb;   // tiles of one worker (CTA or CTA pair)
     gp.num_kb = (c->d + kBK - 1) / kBK;
-    const uint32_t stage_bytes = GemmSmemLayout::a_bytes() + GemmSmemLayout::b_bytes(BN);
+    const uint32_t stage_bytes = GemmSmemLayout::a_bytes() + GemmSmemLayout::b_bytes(b_rows);
     int stages = static_cast<int>((static_cast<uint32_t>(c->max_smem_optin) - 1024 - GemmSmemLayout::misc_bytes()) / stage_bytes);
     stages = std::max(2, std::min(stages, kMaxStages));
     gp.stages = stages;
@@ -299,16 +309,32 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;
-    const int grid = std::min(gp.num_tiles, c->num_sms);
-    const size_t smem = GemmSmemLayout::total(BN, stages);
+    const int workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
+    const int grid = pair ? 2 * workers : workers;
+    const size_t smem = GemmSmemLayout::total(b_rows, stages);
     const bool prof = c->prof_on && c->prof_n < kProfMax;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
-    if (a->logits_out) {
-        if (c->use_cand) cfgms_head_gemm_kernel<true, true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
-        else cfgms_head_gemm_kernel<true, false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
-    } else {
-        if (c->use_cand) cfgms_head_gemm_kernel<false, true><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
-        else cfgms_head_gemm_kernel<false, false><<<grid, kGemmThreads, smem, st>>>(c->tmap_w, c->tmap_h, gp);
+    {
+        using KernelFn = void (*)(const CUtensorMap, const CUtensorMap, const GemmParams);
+        static const KernelFn table[8] = {
+            cfgms_head_gemm_kernel<false, false, false>, cfgms_head_gemm_kernel<true, false, false>,
+            cfgms_head_gemm_kernel<false, true, false>,  cfgms_head_gemm_kernel<true, true, false>,
+            cfgms_head_gemm_kernel<false, false, true>,  cfgms_head_gemm_kernel<true, false, true>,
+            cfgms_head_gemm_kernel<false, true, true>,   cfgms_head_gemm_kernel<true, true, true>};
+        const KernelFn fn = table[(a->logits_out ? 1 : 0) | (c->use_cand ? 2 : 0) | (pair ? 4 : 0)];
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3(static_cast<unsigned>(grid));
+        lc.blockDim = dim3(kGemmThreads);
+        lc.dynamicSmemBytes = smem;
+        lc.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = pair ? 2 : 1;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        lc.attrs = attr;
+        lc.numAttrs = 1;
+        if (cudaLaunchKernelEx(&lc, fn, c->tmap_w, c->tmap_h, gp) != cudaSuccess) return CFGMS_ERR_CUDA;
     }
     ++launches;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 1], st);
@@ -344,6 +370,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
 
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
+    c->info.cta_pair = pair ? 1 : 0;
     c->info.launches_last_step = launches;
     c->info.launches_total += launches;
     c->info.h2d_bytes_last_step = 0; c->info.d2h_bytes_last_step = 0;

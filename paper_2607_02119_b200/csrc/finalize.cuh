@@ -344,9 +344,10 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
 // V/8 values K1's epilogue emitted (top-4 of every 32-token chunk, descending) instead of all V
 // logits.  Lane l keeps chunks l, l+32, ... in registers.
 //   t_E = k-th largest emitted value  <=  true threshold (the emitted set is a subset);
-//   a chunk whose 4th emitted value is < t_E cannot hide anything >= t_E, so its emitted values
-//   >= t_E are all of its candidates; a chunk whose 4th value reaches t_E ("overflow", rare) is
-//   re-read in full from the z spill.  The candidate set {z >= t_E} is then complete and the
+//   K1 selects with 27-bit key buckets, so a value it did NOT emit has
+//   float_key(hidden) <= float_key(smallest emitted) | 31: a chunk with (key4 | 31) < t_E cannot
+//   hide anything >= t_E and its emitted values >= t_E are all of its candidates; a chunk whose
+//   bound reaches t_E ("overflow") is re-read in full from the z spill.  The candidate set {z >= t_E} is then complete and the
 //   exact threshold is its k-th largest (= t_E when no chunk overflowed).
 // t_E itself: with j = ceil(k / G), lo = min over chunks of their j-th value is a lower bound
 // (G*j >= k values are >= lo); ONE histogram pass with 256 linear buckets over [lo, max] finds
@@ -402,9 +403,10 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
         const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
         const float temp = p.temp[r];
-        const int tk = p.top_k[r];
-        const bool greedy = (tk == 1) || (temp == 0.f);
-        const bool filter = !greedy && tk > 0 && tk < V;
+        const int tk_raw = p.top_k[r];
+        const bool greedy = (tk_raw == 1) || (temp == 0.f);
+        const bool filter = !greedy && tk_raw > 0 && tk_raw < V;
+        const int tk = greedy ? 1 : tk_raw;   // greedy = exact top-1 (ties: lowest token), no noise
         const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
         BestSV best = {-INFINITY, 0x7fffffff};
 
@@ -424,13 +426,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     key[j][0] = key[j][1] = key[j][2] = key[j][3] = 0u;
                 }
             }
-            if (greedy) {
-                // argmax = best chunk maximum; inside a chunk the emitted maximum is its lowest-index one
-#pragma unroll
-                for (int j = 0; j < CPL; ++j)
-                    if (j * 32 + lane < G)
-                        best_update(best, key_float(key[j][0]), (j * 32 + lane) * 32 + static_cast<int>(src[j] & 31u));
-            } else {
+            {
                 // ---- t_E: k-th largest of the E emitted values
                 const int jj = (tk + G - 1) / G - 1;           // 0..3: the (jj+1)-th value of every chunk
                 uint32_t lo = 0xffffffffu, hi = 0u;
@@ -518,7 +514,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
 #pragma unroll
                 for (int j = 0; j < CPL; ++j) {
                     const int c = j * 32 + lane;
-                    const bool ovf = c < G && key[j][3] >= tE;
+                    const bool ovf = c < G && (key[j][3] | 31u) >= tE;
                     any_overflow |= __ballot_sync(0xffffffffu, ovf);
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
@@ -537,7 +533,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     int n_new = 0;   // values >= t_E that were hidden behind a chunk's four emitted ones
 #pragma unroll
                     for (int j = 0; j < CPL; ++j) {
-                        uint32_t ovf_mask = __ballot_sync(0xffffffffu, j * 32 + lane < G && key[j][3] >= tE);
+                        uint32_t ovf_mask = __ballot_sync(0xffffffffu, j * 32 + lane < G && (key[j][3] | 31u) >= tE);
                         while (ovf_mask && n_list >= 0) {
                             const int cc = j * 32 + __ffs(ovf_mask) - 1;
                             ovf_mask &= ovf_mask - 1u;
@@ -587,7 +583,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                         const uint32_t ck = list_key[e];
                         if (ck >= thr) {
                             const int v = list_v[e];
-                            best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                            best_update(best, greedy ? key_float(ck) : key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
                         }
                     }
                 } else {
@@ -595,7 +591,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     for (int v = lane; v < V; v += 32) {
                         const float zv = __ldg(zr + v);
                         if (float_key(zv) >= thr_full)
-                            best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                            best_update(best, greedy ? zv + 0.0f : zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
                     }
                 }
             }

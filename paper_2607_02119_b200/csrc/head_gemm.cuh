@@ -1,5 +1,5 @@
-// K1 — head projection + CFG merge + temperature (rows a1-a2 and the first part of a3 of
-// DESIGN.md's hot-path table; Eq. 1).
+// K1 — head projection + CFG merge + temperature + per-chunk candidate pass (rows a1-a2 and
+// the first part of a3 of DESIGN.md's hot-path table; Eq. 1).
 //
 // Orientation ("swap-AB", B200-first): the head weights are the M operand and the batch rows
 // are the N operand of tcgen05.mma, so one accumulator tile is
@@ -10,31 +10,45 @@
 //   * the cond row and its uncond companion are ADJACENT TMEM COLUMNS, i.e. adjacent registers
 //     of the same thread after tcgen05.ld: Eq. 1 is two FMAs per merged logit, no shuffles;
 //   * per-token bias (W_i e_i, folded at create) is one scalar per thread;
+//   * an epilogue warp owns 32 consecutive tokens (its TMEM lane quarter) = exactly one
+//     candidate chunk, so the chunk's selection needs no cross-warp traffic;
 //   * the z spill is written with 32 consecutive tokens per warp store (128 B coalesced).
 //
-// Warp roles (192 threads, persistent over tiles, 1 CTA/SM):
-//   warp 0      TMA producer: W tile [128 x 64] + H tile [BN x 64] bf16 -> 128B-swizzled smem ring
-//   warp 1      TMEM allocator + single-thread tcgen05.mma issuer (M=128, N=BN, K=16), 2 accumulator
-//               stages in TMEM so the epilogue of tile t overlaps the mainloop of tile t+1
-//   warps 2-5   epilogue: tcgen05.ld -> merge -> x 1/temp -> z[row][n] (fp32) (+ debug tap)
+// kPair: two CTAs of a cluster (same TPC) run ONE tcgen05.mma.cta_group::2 of M = 256: each CTA
+// brings its own 128-token weight tile and HALF of the batch-row tile, which halves the
+// shared-memory fill and read traffic of the row operand (the limiter of the one-CTA kernel at
+// large batches).  Each CTA's epilogue reads its own 128 accumulator lanes from its own TMEM.
+//
+// Warp roles (320 threads, persistent over tiles, 1 CTA/SM):
+//   warp 0      TMA producer: W tile [128 x 64] + H tile [BN (or BN/2) x 64] bf16 -> 128B-swizzled ring
+//   warp 1      TMEM allocator + single-thread tcgen05.mma issuer (leader CTA only when kPair),
+//               2 accumulator stages in TMEM so the epilogue of tile t overlaps the mainloop of t+1
+//   warps 2-9   epilogue, two warps per TMEM lane quarter (alternate 64-column slab pairs):
+//               tcgen05.ld -> merge -> x 1/temp -> z spill (fp32) -> per-chunk top-4 candidates
 #pragma once
 #include "ptx_sm100.cuh"
 
 namespace cfgms {
 
-constexpr int kBM = 128;        // vocabulary rows per tile (UMMA M)
+constexpr int kBM = 128;        // vocabulary rows per CTA tile (UMMA M, or half of M = 256 when paired)
 constexpr int kBK = 64;         // K elements per stage (128 B = swizzle span)
 constexpr int kMaxBN = 256;     // batch rows per tile (UMMA N)
-constexpr int kGemmThreads = 192;
+constexpr int kEpiWarps = 8;
+constexpr int kGemmThreads = 64 + 32 * kEpiWarps;
 constexpr int kMaxStages = 8;
 constexpr int kTmemCols = 512;
+constexpr int kCoefSlots = 512; // two-row slots whose coefficients fit the shared-memory table (R <= 1024)
+constexpr int kStgPitch = 33;   // words; +1 keeps both access patterns of the transpose conflict-free
 
-// Per two-row slot coefficients: out0 = c00*acc[2j] + c01*acc[2j+1] + bias*d0 (request at the
-// even row), out1 = c11*acc[2j+1] + bias*d1 (only when the slot holds two unpaired rows).
-struct __align__(16) SlotCoef {
-    float c00, c01, d0, c11;
-    float d1, m00, m01;       // m00/m01: pre-temperature merge weights for the debug tap
+// Per two-row slot: out0 = c00*acc[2j] + c01*acc[2j+1] + bias*d0 (request at the even row);
+// out1 = c11*acc[2j+1] + bias*d1 (only when the slot holds two unpaired rows).
+struct __align__(16) SlotCoefA {
+    float c00, c01, d0;
     int kind;                 // bit0: even row owns a request; bit1: odd row owns its own request
+};
+struct __align__(16) SlotCoefB {
+    float c11, d1;
+    float m00, m01;           // pre-temperature merge weights for the debug tap
 };
 
 struct GemmParams {
@@ -45,67 +59,125 @@ struct GemmParams {
     const float* bias;   // [NT]
     float* z;            // [R][NT]
     float* tap;          // nullable [R][NT]
-    float* cand_val;     // nullable [R][NT/32][4]: top-4 z of every 32-token chunk, descending
-    uint32_t* cand_src;  // nullable [R][NT/32]: their lane offsets inside the chunk, 8 bits each
+    float* cand_val;     // nullable [R][NT/32][4]: four z of every 32-token chunk, descending (see below)
+    uint32_t* cand_src;  // nullable [R][NT/32]: their token offsets inside the chunk, 8 bits each
     int* err;            // sticky error word {code | row << 8}
     uint64_t policy_w, policy_h;
 };
 
 struct GemmSmemLayout {
-    // dynamic smem (1024-aligned): A ring | B ring | coefficients | barriers | tmem ptr
+    // dynamic smem (1024-aligned): A ring | B ring | coefA | coefB | barriers | candidate transpose
     __host__ __device__ static constexpr uint32_t a_bytes() { return kBM * kBK * 2; }
-    __host__ __device__ static constexpr uint32_t b_bytes(int BN) { return static_cast<uint32_t>(BN) * kBK * 2; }
-    __host__ __device__ static constexpr uint32_t coef_bytes() { return (kMaxBN / 2) * sizeof(SlotCoef); }
-    __host__ __device__ static constexpr uint32_t stage_bytes() { return 32 * (kBM + 1) * 4; }  // candidate transpose
-    __host__ __device__ static constexpr uint32_t misc_bytes() { return coef_bytes() + 256 + stage_bytes(); }
-    __host__ __device__ static constexpr uint32_t total(int BN, int stages) {
-        return 1024 + stages * (a_bytes() + b_bytes(BN)) + misc_bytes();
+    __host__ __device__ static constexpr uint32_t b_bytes(int rows) { return static_cast<uint32_t>(rows) * kBK * 2; }
+    __host__ __device__ static constexpr uint32_t coef_bytes() { return kCoefSlots * (sizeof(SlotCoefA) + sizeof(SlotCoefB)); }
+    __host__ __device__ static constexpr uint32_t stg_bytes() { return kEpiWarps * 32 * kStgPitch * 4; }
+    __host__ __device__ static constexpr uint32_t misc_bytes() { return coef_bytes() + 256 + stg_bytes(); }
+    __host__ __device__ static constexpr uint32_t total(int b_rows, int stages) {
+        return 1024 + stages * (a_bytes() + b_bytes(b_rows)) + misc_bytes();
     }
 };
 
-// Per-chunk candidate pass (north_star step 3, "per-N-tile top-k candidate pass held in
-// registers").  In this orientation a thread owns ONE token and many requests, the wrong axis
-// for a per-request top-k, so every 32-column accumulator slab is transposed through a 16 KB
-// shared-memory stage: afterwards epilogue thread (o, q) owns output column o (one request)
-// and the 32 tokens of vocabulary chunk q of the tile, and keeps the chunk's four largest z
-// (descending, lowest token first among equals) in registers with plain compares/selects.
-constexpr int kStageCols = 32;                 // output columns staged per round
-constexpr int kStagePitch = kBM + 1;           // words; +1 keeps both access patterns conflict-free
-__device__ __forceinline__ void top4_insert(float x, int e, float (&t)[4], int (&ix)[4]) {
-    const bool c0 = x > t[0], c1 = x > t[1], c2 = x > t[2], c3 = x > t[3];
-    t[3] = c2 ? t[2] : (c3 ? x : t[3]);   ix[3] = c2 ? ix[2] : (c3 ? e : ix[3]);
-    t[2] = c1 ? t[1] : (c2 ? x : t[2]);   ix[2] = c1 ? ix[1] : (c2 ? e : ix[2]);
-    t[1] = c0 ? t[0] : (c1 ? x : t[1]);   ix[1] = c0 ? ix[0] : (c1 ? e : ix[1]);
-    t[0] = c0 ? x : t[0];                 ix[0] = c0 ? e : ix[0];
+// Slot coefficients from pair_map / w / temp (DESIGN.md batch layout contract).
+__device__ __forceinline__ void make_slot_coef(const GemmParams& p, int r0, SlotCoefA& a, SlotCoefB& b) {
+    a = {0.f, 0.f, 0.f, 0};
+    b = {0.f, 0.f, 0.f, 0.f};
+    const int r1 = r0 + 1;
+    if (r0 >= p.R) return;
+    const int pm0 = p.pair_map[r0];
+    const int pm1 = r1 < p.R ? p.pair_map[r1] : -1;
+    const float t0 = p.temp[r0];
+    const float it0 = t0 == 0.f ? 1.f : 1.f / t0;
+    if (pm0 == r1 && pm1 == r0) {                       // (cond, uncond) pair: Eq. 1
+        const float w = p.w[r0];
+        a.c00 = w * it0; a.c01 = (1.f - w) * it0; a.d0 = it0; a.kind = 1;
+        b.m00 = w; b.m01 = 1.f - w;
+    } else if (pm0 == -1 && pm1 == -1) {                // two unpaired rows
+        a.c00 = it0; a.d0 = it0; a.kind = 1;
+        b.m00 = 1.f;
+        if (r1 < p.R) {
+            const float t1 = p.temp[r1];
+            const float it1 = t1 == 0.f ? 1.f : 1.f / t1;
+            b.c11 = it1; b.d1 = it1;
+            a.kind = 3;
+        }
+    } else {                                            // contract violated
+        atomicCAS(p.err, 0, 3 /* CFGMS_ERR_LAYOUT */ | (r0 << 8));
+    }
 }
 
-template <bool kTap, bool kCand>
+// Per-chunk candidate pass (north_star step 3, "per-N-tile top-k candidate pass held in warp
+// registers").  The warp's 32 tokens x 32 requests block is transposed through a warp-private
+// shared-memory stage; afterwards lane o owns request o and the chunk's 32 z values.  It keeps
+// the four largest as PACKED keys (order-preserving 27-bit float key | 5-bit reversed token
+// offset) with 7 integer min/max per value — no predicates, no index bookkeeping — then
+// re-reads the four exact values and emits them sorted (descending, lowest token first).
+// Selection granularity is the 27-bit key bucket: a value that is NOT emitted has
+//     float_key(hidden) <= float_key(smallest emitted) | 31,
+// which is the bound K2 uses to decide whether a chunk may hide a top-k member.
+__device__ __forceinline__ void chunk_top4(const float* col, float (&val)[4], uint32_t& src) {
+    uint32_t t0 = 0u, t1 = 0u, t2 = 0u, t3 = 0u;
+#pragma unroll
+    for (int e = 0; e < 32; ++e) {
+        const uint32_t u = __float_as_uint(col[e]);
+        const uint32_t s = static_cast<uint32_t>(static_cast<int32_t>(u) >> 31);
+        uint32_t pk = ((u ^ (s | 0x80000000u)) | 31u) ^ static_cast<uint32_t>(e);
+        uint32_t m;
+        m = min(t0, pk); t0 = max(t0, pk); pk = m;
+        m = min(t1, pk); t1 = max(t1, pk); pk = m;
+        m = min(t2, pk); t2 = max(t2, pk); pk = m;
+        t3 = max(t3, pk);
+    }
+    int ix[4] = {static_cast<int>((t0 & 31u) ^ 31u), static_cast<int>((t1 & 31u) ^ 31u),
+                 static_cast<int>((t2 & 31u) ^ 31u), static_cast<int>((t3 & 31u) ^ 31u)};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) val[j] = col[ix[j]];
+    // exact order inside a bucket: value descending, token ascending (5-comparator network)
+#define CFGMS_CX(a, b)                                                                   \
+    {                                                                                    \
+        const bool sw = (val[b] > val[a]) || (val[b] == val[a] && ix[b] < ix[a]);        \
+        const float tv = sw ? val[b] : val[a]; val[b] = sw ? val[a] : val[b]; val[a] = tv; \
+        const int ti = sw ? ix[b] : ix[a];    ix[b] = sw ? ix[a] : ix[b];    ix[a] = ti; \
+    }
+    CFGMS_CX(0, 1) CFGMS_CX(2, 3) CFGMS_CX(0, 2) CFGMS_CX(1, 3) CFGMS_CX(1, 2)
+#undef CFGMS_CX
+    src = static_cast<uint32_t>(ix[0]) | (static_cast<uint32_t>(ix[1]) << 8) | (static_cast<uint32_t>(ix[2]) << 16) |
+          (static_cast<uint32_t>(ix[3]) << 24);
+}
+
+template <bool kTap, bool kCand, bool kPair>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
                        const GemmParams p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const int stages = p.stages;
+    const int BN = p.BN;
+    const int b_rows = kPair ? BN / 2 : BN;          // batch rows this CTA stages per K block
     const uint32_t a_bytes = GemmSmemLayout::a_bytes();
-    const uint32_t b_bytes = GemmSmemLayout::b_bytes(p.BN);
+    const uint32_t b_bytes = GemmSmemLayout::b_bytes(b_rows);
     const uint32_t smem_a = smem_base;
     const uint32_t smem_b = smem_a + stages * a_bytes;
-    const uint32_t smem_coef = smem_b + stages * b_bytes;
-    const uint32_t bar_base = smem_coef + GemmSmemLayout::coef_bytes();
-    // barriers: full[stages], empty[stages], tmem_full[2], tmem_empty[2]  (8 B each)
+    const uint32_t smem_coef_a = smem_b + stages * b_bytes;
+    const uint32_t smem_coef_b = smem_coef_a + kCoefSlots * sizeof(SlotCoefA);
+    const uint32_t bar_base = smem_coef_b + kCoefSlots * sizeof(SlotCoefB);
+    // barriers: full[8] | empty[8] | tmem_full[2] | tmem_empty[2] | tmem base pointer   (8 B each)
     const uint32_t bar_full = bar_base;
     const uint32_t bar_empty = bar_base + 8 * kMaxStages;
     const uint32_t bar_tfull = bar_base + 16 * kMaxStages;
     const uint32_t bar_tempty = bar_tfull + 16;
     const uint32_t tmem_ptr_smem = bar_tempty + 16;
-    const uint32_t smem_stage = bar_base + 256;
+    const uint32_t smem_stg = bar_base + 256;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    SlotCoef* coef = reinterpret_cast<SlotCoef*>(smem_gen + (smem_coef - smem_base));
+    SlotCoefA* coef_a = reinterpret_cast<SlotCoefA*>(smem_gen + (smem_coef_a - smem_base));
+    SlotCoefB* coef_b = reinterpret_cast<SlotCoefB*>(smem_gen + (smem_coef_b - smem_base));
     volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + (tmem_ptr_smem - smem_base));
-    float* stage = reinterpret_cast<float*>(smem_gen + (smem_stage - smem_base));
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+    const uint32_t cta_rank = kPair ? cluster_ctarank() : 0u;
+    const bool leader = cta_rank == 0u;
+    const int worker = kPair ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
+    const int num_workers = kPair ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmap_w);
@@ -116,170 +188,210 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
         }
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
-            mbar_init(bar_tempty + 8 * a, 4);
+            mbar_init(bar_tempty + 8 * a, kEpiWarps * (kPair ? 2 : 1));
         }
         fence_barrier_init();
     }
     if (warp == 1) {
-        tmem_alloc(tmem_ptr_smem, kTmemCols);
-        tmem_relinquish();
+        if (kPair) { tmem_alloc_pair(tmem_ptr_smem, kTmemCols); tmem_relinquish_pair(); }
+        else { tmem_alloc(tmem_ptr_smem, kTmemCols); tmem_relinquish(); }
     }
     tc_fence_before();
-    __syncthreads();
+    if (kPair) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
 
-    const int BN = p.BN;
     if (warp == 0) {
-        // ================= TMA producer =================
-        if (lane == 0) {
-            int s = 0;
-            uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
-                const int rb = tile % p.num_row_blocks;
-                const int vt = tile / p.num_row_blocks;
-                for (int kb = 0; kb < p.num_kb; ++kb) {
-                    mbar_wait(bar_empty + 8 * s, phase ^ 1, p.err, 1);
-                    mbar_arrive_expect_tx(bar_full + 8 * s, a_bytes + b_bytes);
-                    tma_load_2d(smem_a + s * a_bytes, &tmap_w, bar_full + 8 * s, kb * kBK, vt * kBM, p.policy_w);
-                    tma_load_2d(smem_b + s * b_bytes, &tmap_h, bar_full + 8 * s, kb * kBK, rb * BN, p.policy_h);
-                    if (++s == stages) { s = 0; phase ^= 1; }
+        // ================= TMA producer (every CTA) =================
+        // The whole warp walks the loop (warp-uniform state stays in uniform registers); one
+        // elected lane issues.  Transaction bytes of both CTAs land on the leader's barrier.
+        const uint32_t full_sig = kPair ? mapa_shared(bar_full, 0u) : bar_full;
+        const uint32_t tx_bytes = (a_bytes + b_bytes) * (kPair ? 2u : 1u);
+        int s = 0;
+        uint32_t phase = 0;
+        for (int tile = worker; tile < p.num_tiles; tile += num_workers) {
+            const int rb = tile % p.num_row_blocks;
+            const int vp = tile / p.num_row_blocks;
+            const int vt = kPair ? vp * 2 + static_cast<int>(cta_rank) : vp;
+            const int row0 = rb * BN + static_cast<int>(cta_rank) * b_rows;
+            for (int kb = 0; kb < p.num_kb; ++kb) {
+                mbar_wait(bar_empty + 8 * s, phase ^ 1, p.err, 1);
+                if (elect_one()) {
+                    if (leader) mbar_arrive_expect_tx(bar_full + 8 * s, tx_bytes);
+                    if (kPair) {
+                        tma_load_2d_pair(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
+                        tma_load_2d_pair(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
+                    } else {
+                        tma_load_2d(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
+                        tma_load_2d(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
+                    }
                 }
+                __syncwarp();
+                if (++s == stages) { s = 0; phase ^= 1; }
             }
         }
-        __syncwarp();
     } else if (warp == 1) {
-        // ================= MMA issuer =================
-        if (lane == 0) {
-            const uint32_t idesc = umma_idesc_bf16_f32(kBM, BN);
+        // ================= MMA issuer (leader CTA) =================
+        // This loop paces the tensor pipe: 4 MMAs of 128 cycles per K block, so it must stay far
+        // below 512 cycles per iteration — whole-warp control flow, one elected lane issues.
+        if (leader) {
+            const uint32_t idesc = umma_idesc_bf16_f32(kPair ? 2 * kBM : kBM, BN);
+            const uint64_t a_desc0 = umma_smem_desc_sw128(smem_a);
+            const uint64_t b_desc0 = umma_smem_desc_sw128(smem_b);
             int s = 0;
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
-            for (int tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+            for (int tile = worker; tile < p.num_tiles; tile += num_workers) {
                 mbar_wait(bar_tempty + 8 * acc, acc_phase ^ 1, p.err, 2);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * BN;
                 for (int kb = 0; kb < p.num_kb; ++kb) {
                     mbar_wait(bar_full + 8 * s, phase, p.err, 3);
                     tc_fence_after();
-                    const uint64_t a_desc = umma_smem_desc_sw128(smem_a + s * a_bytes);
-                    const uint64_t b_desc = umma_smem_desc_sw128(smem_b + s * b_bytes);
+                    if (elect_one()) {
+                        // the start-address field counts 16-byte units
+                        const uint64_t a_desc = a_desc0 + static_cast<uint64_t>((s * a_bytes) >> 4);
+                        const uint64_t b_desc = b_desc0 + static_cast<uint64_t>((s * b_bytes) >> 4);
 #pragma unroll
-                    for (int k = 0; k < kBK / 16; ++k) {
-                        // advance 16 bf16 = 32 B along K inside the swizzle span: +2 in the >>4 field
-                        umma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                        for (int k = 0; k < kBK / 16; ++k) {
+                            // advance 16 bf16 = 32 B along K inside the swizzle span: +2 in the >>4 field
+                            if (kPair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                            else umma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                        }
+                        if (kPair) umma_commit_pair(bar_empty + 8 * s); else umma_commit(bar_empty + 8 * s);
+                        if (kb == p.num_kb - 1) {
+                            if (kPair) umma_commit_pair(bar_tfull + 8 * acc); else umma_commit(bar_tfull + 8 * acc);
+                        }
                     }
-                    umma_commit(bar_empty + 8 * s);
+                    __syncwarp();
                     if (++s == stages) { s = 0; phase ^= 1; }
                 }
-                umma_commit(bar_tfull + 8 * acc);
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
             }
         }
-        __syncwarp();
     } else {
-        // ================= epilogue (warps 2..5) =================
+        // ================= epilogue (warps 2..9, every CTA) =================
+        const int ew = warp - 2;
         const int quarter = warp & 3;             // TMEM lane quarter this warp may read
-        const int et = (warp - 2) * 32 + lane;    // 0..127 index among epilogue threads
+        const int half = ew >> 2;                 // which slab pairs (alternating) this warp takes
+        const int et = ew * 32 + lane;            // 0..255 among epilogue threads
+        float* stg = reinterpret_cast<float*>(smem_gen + (smem_stg - smem_base)) + ew * (32 * kStgPitch);
+        const int nsp = BN / 64;                  // 64-column slab pairs per tile
+        const int slots_per_rb = BN / 2;
+        const bool full_table = p.num_row_blocks * slots_per_rb <= kCoefSlots;
+        const uint32_t tempty_sig = (kPair && !leader) ? mapa_shared(bar_tempty, 0u) : bar_tempty;
+        const size_t NT = static_cast<size_t>(p.NT);
+        if (full_table) {
+            // coefficients of every slot, once (the first mainloop hides it)
+            for (int slot = et; slot < p.num_row_blocks * slots_per_rb; slot += 32 * kEpiWarps) {
+                SlotCoefA ca; SlotCoefB cb;
+                make_slot_coef(p, 2 * slot, ca, cb);
+                coef_a[slot] = ca; coef_b[slot] = cb;
+            }
+            named_bar_sync(1, 32 * kEpiWarps);
+        }
         int acc = 0;
         uint32_t acc_phase = 0;
         int cur_rb = -1;
-        for (int tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        for (int tile = worker; tile < p.num_tiles; tile += num_workers) {
             const int rb = tile % p.num_row_blocks;
-            const int vt = tile / p.num_row_blocks;
-            if (rb != cur_rb) {
-                // slot coefficients of this row block: one slot per epilogue thread
-                named_bar_sync(1, 128);           // everyone finished reading the old table
-                const int slot = et;
-                if (slot < BN / 2) {
-                    const int r0 = rb * BN + 2 * slot, r1 = r0 + 1;
-                    SlotCoef c = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0};
-                    if (r0 < p.R) {
-                        const int pm0 = p.pair_map[r0];
-                        const int pm1 = r1 < p.R ? p.pair_map[r1] : -1;
-                        const float t0 = p.temp[r0];
-                        const float it0 = t0 == 0.f ? 1.f : 1.f / t0;
-                        if (pm0 == r1 && pm1 == r0) {                       // (cond, uncond) pair: Eq. 1
-                            const float w = p.w[r0];
-                            c.c00 = w * it0; c.c01 = (1.f - w) * it0; c.d0 = it0;
-                            c.m00 = w; c.m01 = 1.f - w;
-                            c.kind = 1;
-                        } else if (pm0 == -1 && pm1 == -1) {                // two unpaired rows
-                            c.c00 = it0; c.d0 = it0; c.m00 = 1.f;
-                            c.kind = 1;
-                            if (r1 < p.R) {
-                                const float t1 = p.temp[r1];
-                                const float it1 = t1 == 0.f ? 1.f : 1.f / t1;
-                                c.c11 = it1; c.d1 = it1;
-                                c.kind = 3;
-                            }
-                        } else {                                            // contract violated
-                            atomicCAS(p.err, 0, 3 /* CFGMS_ERR_LAYOUT */ | (r0 << 8));
-                        }
-                    }
-                    coef[slot] = c;
+            const int vp = tile / p.num_row_blocks;
+            const int vt = kPair ? vp * 2 + static_cast<int>(cta_rank) : vp;
+            if (!full_table && rb != cur_rb) {
+                named_bar_sync(1, 32 * kEpiWarps);    // everyone finished reading the old table
+                if (et < slots_per_rb) {
+                    SlotCoefA ca; SlotCoefB cb;
+                    make_slot_coef(p, rb * BN + 2 * et, ca, cb);
+                    coef_a[et] = ca; coef_b[et] = cb;
                 }
-                named_bar_sync(1, 128);
+                named_bar_sync(1, 32 * kEpiWarps);
                 cur_rb = rb;
             }
-            const int n = vt * kBM + quarter * 32 + lane;
+            const int slot_base = full_table ? rb * slots_per_rb : 0;
+            const int nb = vt * kBM + quarter * 32;       // first token of this warp's chunk
+            const int n = nb + lane;
             const bool n_ok = n < p.NT;
+            const bool chunk_ok = nb < p.NT;              // NT % 32 == 0 on the candidate path
             const float bias = n_ok ? __ldg(p.bias + n) : 0.f;
 
             mbar_wait(bar_tfull + 8 * acc, acc_phase, p.err, 4);
             tc_fence_after();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * BN;
-            const int nchunks = BN / 32;
-            for (int c = 0; c < nchunks; ++c) {
-                uint32_t v[32];
-                tmem_ld_32x32b_x32(taddr + c * 32, v);
+            if (half >= nsp) {                            // nothing to read for this warp: release at once
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) { if (kPair && !leader) mbar_arrive_cluster(tempty_sig + 8 * acc); else mbar_arrive(bar_tempty + 8 * acc); }
+            }
+            for (int sp = half; sp < nsp; sp += 2) {
+                uint32_t v[64];
+                tmem_ld_32x32b_x32(taddr + sp * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+                tmem_ld_32x32b_x32(taddr + sp * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
                 tmem_ld_wait();
-                if (c == nchunks - 1) {
-                    // accumulator stage fully read into registers: hand it back to the MMA warp
+                if (sp + 2 >= nsp) {
+                    // this warp's share of the accumulator stage is in registers: hand it back
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_tempty + 8 * acc);
+                    if (lane == 0) { if (kPair && !leader) mbar_arrive_cluster(tempty_sig + 8 * acc); else mbar_arrive(bar_tempty + 8 * acc); }
                 }
-                const int row_base = rb * BN + c * 32;
+                const int row_base = rb * BN + sp * 64;
+                const SlotCoefA* ca = coef_a + slot_base + sp * 32;
+                const SlotCoefB* cb = coef_b + slot_base + sp * 32;
+                float* zp = p.z + static_cast<size_t>(row_base) * NT + n;
+                float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
+                int any_odd = 0;
+                // ---- pass A: the request at the even row of every slot
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const SlotCoef sc = coef[c * 16 + j];
+                for (int j = 0; j < 32; ++j) {
+                    const SlotCoefA c = ca[j];
                     const float a0 = __uint_as_float(v[2 * j]);
                     const float a1 = __uint_as_float(v[2 * j + 1]);
-                    const int r0 = row_base + 2 * j;
-                    const int kind = sc.kind;
-                    if (n_ok && (kind & 1)) {
-                        const float z0 = fmaf(sc.c00, a0, fmaf(sc.c01, a1, bias * sc.d0));
-                        p.z[static_cast<size_t>(r0) * p.NT + n] = z0;
-                        if (kTap) p.tap[static_cast<size_t>(r0) * p.NT + n] = fmaf(sc.m00, a0, fmaf(sc.m01, a1, bias));
-                        if (kCand) stage[(2 * j) * kStagePitch + quarter * 32 + lane] = z0 + 0.0f;
+                    const float z0 = fmaf(c.c00, a0, fmaf(c.c01, a1, bias * c.d0));
+                    const bool own = n_ok && (c.kind & 1);
+                    any_odd |= c.kind;
+                    if (own) {
+                        zp[static_cast<size_t>(2 * j) * NT] = z0;
+                        if (kTap) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
                     }
-                    if (n_ok && (kind & 2)) {
-                        const float z1 = fmaf(sc.c11, a1, bias * sc.d1);
-                        p.z[static_cast<size_t>(r0 + 1) * p.NT + n] = z1;
-                        if (kTap) p.tap[static_cast<size_t>(r0 + 1) * p.NT + n] = a1 + bias;
-                        if (kCand) stage[(2 * j + 1) * kStagePitch + quarter * 32 + lane] = z1 + 0.0f;
-                    }
+                    if (kCand) stg[j * kStgPitch + lane] = own ? z0 + 0.0f : -INFINITY;
                 }
                 if (kCand) {
-                    named_bar_sync(2, 128);                 // slab staged by all four epilogue warps
-                    const int o = et & 31;                  // output column of the slab
-                    const int q = et >> 5;                  // vocabulary chunk of the tile
-                    const int kind_o = coef[c * 16 + (o >> 1)].kind;
-                    const int nb = vt * kBM + q * 32;       // first token of the chunk (NT % 32 == 0)
-                    if (((kind_o >> (o & 1)) & 1) && nb < p.NT) {
-                        float t[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-                        int ix[4] = {0, 0, 0, 0};
-                        const float* col = stage + o * kStagePitch + q * 32;
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) top4_insert(col[e], e, t, ix);
-                        const size_t chunk = (static_cast<size_t>(row_base + o) * p.NT + nb) >> 5;
-                        *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(t[0], t[1], t[2], t[3]);
-                        p.cand_src[chunk] = static_cast<uint32_t>(ix[0]) | (static_cast<uint32_t>(ix[1]) << 8) |
-                                            (static_cast<uint32_t>(ix[2]) << 16) | (static_cast<uint32_t>(ix[3]) << 24);
+                    __syncwarp();
+                    if ((ca[lane].kind & 1) && chunk_ok) {
+                        float val[4]; uint32_t src;
+                        chunk_top4(stg + lane * kStgPitch, val, src);
+                        const size_t chunk = (static_cast<size_t>(row_base + 2 * lane) * NT + nb) >> 5;
+                        *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
+                        p.cand_src[chunk] = src;
                     }
-                    named_bar_sync(2, 128);                 // stage may be overwritten
+                    __syncwarp();
+                }
+                // ---- pass B: slots that hold two unpaired rows — the request at the odd row
+                if (any_odd & 2) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const int kind = ca[j].kind;
+                        const SlotCoefB c = cb[j];
+                        const float a1 = __uint_as_float(v[2 * j + 1]);
+                        const float z1 = fmaf(c.c11, a1, bias * c.d1);
+                        const bool own = n_ok && (kind & 2);
+                        if (own) {
+                            zp[static_cast<size_t>(2 * j + 1) * NT] = z1;
+                            if (kTap) tp[static_cast<size_t>(2 * j + 1) * NT] = a1 + bias;
+                        }
+                        if (kCand) stg[j * kStgPitch + lane] = own ? z1 + 0.0f : -INFINITY;
+                    }
+                    if (kCand) {
+                        __syncwarp();
+                        if ((ca[lane].kind & 2) && chunk_ok) {
+                            float val[4]; uint32_t src;
+                            chunk_top4(stg + lane * kStgPitch, val, src);
+                            const size_t chunk = (static_cast<size_t>(row_base + 2 * lane + 1) * NT + nb) >> 5;
+                            *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
+                            p.cand_src[chunk] = src;
+                        }
+                        __syncwarp();
+                    }
                 }
             }
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
@@ -287,10 +399,10 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
     }
 
     tc_fence_before();
-    __syncthreads();
+    if (kPair) cluster_sync_all(); else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        tmem_dealloc(tmem_base, kTmemCols);
+        if (kPair) tmem_dealloc_pair(tmem_base, kTmemCols); else tmem_dealloc(tmem_base, kTmemCols);
     }
 }
 

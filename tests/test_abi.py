@@ -41,7 +41,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(b.cfgms_config) == 32
     assert C.sizeof(b.cfgms_step_args) == 112
     assert b.cfgms_step_args.seed.offset == 48 and b.cfgms_step_args.T_cap.offset == 96
-    assert C.sizeof(b.cfgms_info) == 72
+    assert C.sizeof(b.cfgms_info) == 80
 
 
 def test_create_without_gpu_fails_loudly():
