@@ -57,6 +57,10 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
 
 #define CFGMS_CFG_SINGLE_CTA 4u  /* tuning/debug: never pair CTAs on one M = 256 MMA                */
 #define CFGMS_CFG_CTA_PAIR 8u    /* tuning/debug: always run the head GEMM on CTA pairs (cta_group::2) */
+#define CFGMS_CFG_NO_OVERLAP 16u /* tuning/debug: launch the finalize kernel strictly after the head
+                                    GEMM.  Default: it is launched as a programmatic dependent of the
+                                    GEMM and consumes finished (stream, row block) groups while the
+                                    GEMM is still running (candidate path with V % 128 == 0)        */
 
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
@@ -64,7 +68,8 @@ typedef struct {
     uint32_t flags;
     int32_t row_tile;  /* debug/tuning: batch rows per accumulator tile (multiple of 64,
                           <= 256); 0 = chosen from R and the SM count                           */
-    int32_t reserved[4];
+    int32_t max_stages; /* debug/tuning: cap on the head GEMM's TMA ring depth (0 = as deep as fits)   */
+    int32_t reserved[3];
 } cfgms_config;
 
 /*
@@ -159,7 +164,7 @@ typedef struct {
     int64_t h2d_bytes_last_step;   /* cfgms_step_host only                                      */
     int64_t d2h_bytes_last_step;
     int32_t cta_pair;              /* 1 when the last head GEMM ran on CTA pairs (cta_group::2) */
-    int32_t reserved_;
+    int32_t overlap;               /* 1 when the last finalize launch overlapped the head GEMM  */
 } cfgms_info;
 int cfgms_get_info(cfgms_ctx* ctx, cfgms_info* out);
 
@@ -172,6 +177,15 @@ int cfgms_get_info(cfgms_ctx* ctx, cfgms_info* out);
  */
 int cfgms_profile_enable(cfgms_ctx* ctx, int on);
 int cfgms_profile_read(cfgms_ctx* ctx, double* gemm_ms, double* finalize_ms, int64_t* steps);
+
+/*
+ * Evidence that the finalize kernel really runs beside the head GEMM (cfgms_info.overlap = 1):
+ * *cells_sampled = (request, stream) cells sampled on the overlapped path since the last call,
+ * *cells_waited = how many of them reached their readiness check before the head GEMM had
+ * finished their (stream, row block) group, i.e. while the GEMM was still running.  Both are 0
+ * when the overlap is off.  One small D2H copy (synchronises the device); resets the counters.
+ */
+int cfgms_overlap_stats(cfgms_ctx* ctx, int64_t* cells_waited, int64_t* cells_sampled);
 
 const char* cfgms_strerror(int status);
 /* Library build string: version, arch, compile flags. */

@@ -17,13 +17,14 @@ CFGMS_CFG_PAD_TOKEN = 1
 CFGMS_CFG_NO_CANDIDATES = 2
 CFGMS_CFG_SINGLE_CTA = 4
 CFGMS_CFG_CTA_PAIR = 8
+CFGMS_CFG_NO_OVERLAP = 16
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
           5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
 
 EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
-           "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read"]
+           "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats"]
 
 
 class CfgmsError(RuntimeError):
@@ -34,7 +35,7 @@ class CfgmsError(RuntimeError):
 
 class cfgms_config(C.Structure):
     _fields_ = [("max_rows", C.c_int32), ("pad_token", C.c_int32), ("flags", C.c_uint32),
-                ("row_tile", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("row_tile", C.c_int32), ("max_stages", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 class cfgms_step_args(C.Structure):
@@ -51,7 +52,7 @@ class cfgms_info(C.Structure):
                 ("row_blocks", C.c_int32), ("vocab_tiles", C.c_int32), ("gemm_grid", C.c_int32),
                 ("pipeline_stages", C.c_int32), ("launches_last_step", C.c_int32),
                 ("launches_total", C.c_int64), ("h2d_bytes_last_step", C.c_int64),
-                ("d2h_bytes_last_step", C.c_int64), ("cta_pair", C.c_int32), ("reserved_", C.c_int32)]
+                ("d2h_bytes_last_step", C.c_int64), ("cta_pair", C.c_int32), ("overlap", C.c_int32)]
 
 
 _LIB = None
@@ -85,6 +86,8 @@ def _lib():
         L.cfgms_profile_enable.argtypes = [C.c_void_p, C.c_int]
         L.cfgms_profile_read.restype = C.c_int
         L.cfgms_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.cfgms_overlap_stats.restype = C.c_int
+        L.cfgms_overlap_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.cfgms_strerror.restype = C.c_char_p
         L.cfgms_strerror.argtypes = [C.c_int]
         L.cfgms_version.restype = C.c_char_p
@@ -130,7 +133,7 @@ class Context:
 
     def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
-                 cta_pair: Optional[bool] = None):
+                 cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -140,6 +143,7 @@ class Context:
         cfg = cfgms_config()
         cfg.max_rows = int(max_rows)
         cfg.row_tile = int(row_tile)
+        cfg.max_stages = int(max_stages)
         if pad_token is not None:
             cfg.pad_token = int(pad_token)
             cfg.flags |= CFGMS_CFG_PAD_TOKEN
@@ -147,6 +151,8 @@ class Context:
             cfg.flags |= CFGMS_CFG_NO_CANDIDATES
         if cta_pair is not None:   # tuning: force the one-CTA or the CTA-pair head GEMM
             cfg.flags |= CFGMS_CFG_CTA_PAIR if cta_pair else CFGMS_CFG_SINGLE_CTA
+        if no_overlap:             # tuning: finalize strictly after the head GEMM
+            cfg.flags |= CFGMS_CFG_NO_OVERLAP
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):
@@ -253,6 +259,15 @@ class Context:
         if rc != 0:
             raise CfgmsError(rc, "cfgms_profile_read")
         return float(g.value), float(f.value), int(n.value)
+
+    def overlap_stats(self):
+        """-> (cells that reached their readiness check while the head GEMM was still producing their
+        group, cells sampled on the overlapped path) since the last call; synchronises."""
+        w, n = C.c_int64(), C.c_int64()
+        rc = _lib().cfgms_overlap_stats(self._h, C.byref(w), C.byref(n))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_overlap_stats")
+        return int(w.value), int(n.value)
 
     def info(self) -> dict:
         inf = cfgms_info()

@@ -40,7 +40,7 @@ struct HostStage {  // device staging for the *_host entry points
 struct cfgms_ctx {
     int S = 0, d = 0, V = 0, NT = 0;
     int device = 0, num_sms = 0;
-    int max_rows = 0, pad_token = 0, row_tile_override = 0;
+    int max_rows = 0, pad_token = 0, row_tile_override = 0, max_stages = 0;
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT]
@@ -50,6 +50,9 @@ struct cfgms_ctx {
     bool use_cand = false;            // V % 32 == 0 && V <= 8192
     __nv_bfloat16* hidden_bf16 = nullptr;  // [max_rows][d], used when the caller passes fp32
     int* err = nullptr;               // device: sticky {code | row << 8}
+    int* ready = nullptr;             // device: [S][row blocks] K1 -> K2 tile arrivals, then one `done` counter
+    int ready_words = 0;
+    bool overlap = false;             // K2 as a programmatic dependent of K1 (candidate path, V % 128 == 0)
     EncodeTiledFn encode = nullptr;
     CUtensorMap tmap_w;
     CUtensorMap tmap_h;
@@ -166,6 +169,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     c->max_rows = (cfg && cfg->max_rows > 0) ? cfg->max_rows : 1024;
     c->pad_token = (cfg && (cfg->flags & CFGMS_CFG_PAD_TOKEN)) ? cfg->pad_token : V;
     c->row_tile_override = cfg ? cfg->row_tile : 0;
+    c->max_stages = (cfg && cfg->max_stages >= 2) ? cfg->max_stages : kMaxStages;
     c->pair_mode = (cfg && (cfg->flags & CFGMS_CFG_SINGLE_CTA)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_CTA_PAIR)) ? 2 : 0;
     if (c->row_tile_override < 0 || c->row_tile_override > kMaxBN || (c->row_tile_override % 64) != 0) {
         delete c;
@@ -197,6 +201,15 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
         return rc;
     }
     cudaMemset(c->err, 0, 2 * sizeof(int));
+    c->overlap = c->use_cand && (V % kBM) == 0 && !(cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP));
+    if (c->overlap) {
+        c->ready_words = ((S * ((c->max_rows + 63) / 64) + 1 + 1) & ~1) + 4;   // counters | done | pad | stats (2 x u64)
+        if ((rc = dev_alloc(&c->ready, static_cast<size_t>(c->ready_words))) != CFGMS_OK) {
+            cfgms_destroy(c);
+            return rc;
+        }
+        cudaMemset(c->ready, 0, static_cast<size_t>(c->ready_words) * sizeof(int));
+    }
 
     if ((rc = make_tmap_2d(c, &c->tmap_w, heads, static_cast<uint64_t>(c->NT), static_cast<uint64_t>(d), kBM)) != CFGMS_OK) {
         cfgms_destroy(c);
@@ -254,6 +267,7 @@ void cfgms_destroy(cfgms_ctx* c) {
     cudaFree(c->cand_src);
     cudaFree(c->hidden_bf16);
     cudaFree(c->err);
+    cudaFree(c->ready);
     if (c->prof_ev) {
         for (int j = 0; j < 3 * kProfMax; ++j) cudaEventDestroy(c->prof_ev[j]);
         delete[] c->prof_ev;
@@ -301,11 +315,13 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     gp.num_kb = (c->d + kBK - 1) / kBK;
     const uint32_t stage_bytes = GemmSmemLayout::a_bytes() + GemmSmemLayout::b_bytes(b_rows);
     int stages = static_cast<int>((static_cast<uint32_t>(c->max_smem_optin) - 1024 - GemmSmemLayout::misc_bytes()) / stage_bytes);
-    stages = std::max(2, std::min(stages, kMaxStages));
+    stages = std::max(2, std::min(stages, std::min(kMaxStages, c->max_stages)));
     gp.stages = stages;
     gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp;
     gp.bias = c->bias; gp.z = c->z; gp.tap = a->logits_out; gp.err = c->err;
     gp.cand_val = c->cand_val; gp.cand_src = c->cand_src;
+    gp.ready = c->overlap ? c->ready : nullptr;
+    gp.V = c->V;
     // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;
@@ -348,14 +364,33 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.pad_token = c->pad_token;
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
     fp.cand_val = c->cand_val; fp.cand_src = c->cand_src;
+    fp.ready = gp.ready;
+    fp.done = c->overlap ? c->ready + (c->ready_words - 5) : nullptr;
+    fp.stats = c->overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 4)) : nullptr;
+    fp.err = c->err;
+    fp.BN = BN; fp.num_row_blocks = nrb;
+    fp.ready_target = (c->V / kBM) * kEpiWarps;   // every epilogue warp of every vocabulary tile of the stream
     if (c->use_cand) {
         const size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;
         const int cells = a->R * c->S;
         const int fblocks = (cells + kCandWarps - 1) / kCandWarps;
-        if (c->V <= 1024) cfgms_finalize_cand_kernel<1><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
-        else if (c->V <= 2048) cfgms_finalize_cand_kernel<2><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
-        else if (c->V <= 4096) cfgms_finalize_cand_kernel<4><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
-        else cfgms_finalize_cand_kernel<8><<<fblocks, kCandWarps * 32, fsmem, st>>>(fp);
+        using FinFn = void (*)(const FinalizeParams);
+        const FinFn ffn = c->V <= 1024 ? cfgms_finalize_cand_kernel<1> : c->V <= 2048 ? cfgms_finalize_cand_kernel<2>
+                        : c->V <= 4096 ? cfgms_finalize_cand_kernel<4> : cfgms_finalize_cand_kernel<8>;
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3(static_cast<unsigned>(fblocks));
+        lc.blockDim = dim3(kCandWarps * 32);
+        lc.dynamicSmemBytes = fsmem;
+        lc.stream = st;
+        // Programmatic dependent launch: K2's CTAs are scheduled beside the still-running K1 (which
+        // triggers right after its setup) and wait per cell on the ready counters.  With the profiling
+        // events between the two launches the kernels run back to back instead.
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = attr;
+        lc.numAttrs = (c->overlap && !prof) ? 1 : 0;
+        if (cudaLaunchKernelEx(&lc, ffn, fp) != cudaSuccess) return CFGMS_ERR_CUDA;
     } else {
         const dim3 fgrid(c->S, a->R);
         const size_t fsmem = static_cast<size_t>(c->V) * 8;
@@ -371,6 +406,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
     c->info.cta_pair = pair ? 1 : 0;
+    c->info.overlap = (c->overlap && !prof) ? 1 : 0;
     c->info.launches_last_step = launches;
     c->info.launches_total += launches;
     c->info.h2d_bytes_last_step = 0; c->info.d2h_bytes_last_step = 0;
@@ -472,6 +508,7 @@ int cfgms_last_device_error(cfgms_ctx* c, int32_t* row_out) {
     if (word[0] == 0) return CFGMS_OK;
     if (row_out) *row_out = word[0] >> 8;
     cudaMemset(c->err, 0, sizeof(word));
+    if (c->ready) cudaMemset(c->ready, 0, static_cast<size_t>(c->ready_words - 4) * sizeof(int));   // a failed step may leave them armed
     return word[0] & 0xff;
 }
 
@@ -502,6 +539,19 @@ int cfgms_profile_read(cfgms_ctx* c, double* gemm_ms, double* finalize_ms, int64
     }
     *gemm_ms = g; *finalize_ms = f; *steps = c->prof_n;
     c->prof_n = 0;
+    return CFGMS_OK;
+}
+
+int cfgms_overlap_stats(cfgms_ctx* c, int64_t* cells_waited, int64_t* cells_sampled) {
+    if (!c || !cells_waited || !cells_sampled) return CFGMS_ERR_ARG;
+    *cells_waited = *cells_sampled = 0;
+    if (!c->ready) return CFGMS_OK;
+    unsigned long long w[2] = {0, 0};
+    int* st = c->ready + (c->ready_words - 4);
+    if (cudaMemcpy(w, st, sizeof(w), cudaMemcpyDeviceToHost) != cudaSuccess) return CFGMS_ERR_CUDA;
+    if (cudaMemset(st, 0, sizeof(w)) != cudaSuccess) return CFGMS_ERR_CUDA;
+    *cells_waited = static_cast<int64_t>(w[0]);
+    *cells_sampled = static_cast<int64_t>(w[1]);
     return CFGMS_OK;
 }
 

@@ -17,6 +17,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "ptx_sm100.cuh"
+
 namespace cfgms {
 
 constexpr int kFinThreads = 256;
@@ -38,6 +40,13 @@ struct FinalizeParams {
     int32_t T_cap;
     const float* cand_val;    // [R][NT/32][4]  (candidate path only)
     const uint32_t* cand_src; // [R][NT/32]
+    // Overlap with K1 (candidate path, V % 128 == 0): K1's epilogue warps count finished tiles per
+    // (stream, row block) in ready[]; a cell is consumed once its group reached ready_target.
+    int* ready;               // nullable [S][num_row_blocks]
+    int* done;                // CTAs of this grid that finished; the last one clears ready[] for the next step
+    unsigned long long* stats;// {cells that arrived before their group was complete, cells sampled}
+    int* err;                 // sticky error word
+    int BN, num_row_blocks, ready_target;
 };
 
 // Philox4x32-10 (Salmon et al. 2011): ten rounds of two 32x32->64 multiplies with key bumps.
@@ -357,7 +366,7 @@ constexpr int kCandWarps = 4;
 
 struct GlobalKeys {
     const float* z;
-    __device__ __forceinline__ uint32_t operator()(int e) const { return float_key(__ldg(z + e)); }
+    __device__ __forceinline__ uint32_t operator()(int e) const { return float_key(__ldcg(z + e)); }
 };
 
 __device__ __forceinline__ BestSV warp_argmax(BestSV b) {
@@ -379,12 +388,13 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     extern __shared__ uint32_t dyn[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+    // cells in the order K1 finishes them: stream-major, rows ascending (= row blocks ascending)
     const int cell = blockIdx.x * kCandWarps + warp;
-    if (cell >= p.R * p.S) return;
-    const int r = cell / p.S;
-    const int i = cell - r * p.S;
+    const bool in_range = cell < p.R * p.S;
+    const int i = in_range ? cell / p.R : 0;
+    const int r = in_range ? cell - i * p.R : 0;
     const int pm = p.pair_map[r];
-    if (pm >= 0 && (r & 1)) return;  // companion row
+    const bool valid = in_range && !(pm >= 0 && (r & 1));   // a companion row is written by its cond row
 
     const int V = p.V;
     const int G = V >> 5;            // chunks of this cell
@@ -397,9 +407,28 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     int* list_v = reinterpret_cast<int*>(list_key + cap);
 
     const int tau = p.step[r];
-    const bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    const bool active = valid && (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
     int token = p.pad_token;
     if (active) {
+        if (p.ready) {
+            // wait until K1 has written every tile of this (stream, row block): acquire pairs with
+            // the epilogue warps' red.release; bounded so a pipeline bug fails loudly
+            const int* flag = p.ready + i * p.num_row_blocks + r / p.BN;
+            if (lane == 0) atomicAdd(p.stats + 1, 1ull);
+            if (lane == 0 && ld_acquire_gpu(flag) < p.ready_target) {
+                atomicAdd(p.stats, 1ull);
+                const uint64_t t0 = global_timer_ns();
+                while (ld_acquire_gpu(flag) < p.ready_target) {
+                    __nanosleep(200);
+                    if (global_timer_ns() - t0 > 2000000000ull) {
+                        atomicCAS(p.err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (9 << 8));
+                        __threadfence_system();
+                        __trap();
+                    }
+                }
+            }
+            __syncwarp();
+        }
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
         const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
         const float temp = p.temp[r];
@@ -417,8 +446,8 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
             for (int j = 0; j < CPL; ++j) {
                 const int c = j * 32 + lane;
                 if (c < G) {
-                    const float4 v4 = __ldg(reinterpret_cast<const float4*>(p.cand_val) + chunk0 + c);
-                    src[j] = __ldg(p.cand_src + chunk0 + c);
+                    const float4 v4 = __ldcg(reinterpret_cast<const float4*>(p.cand_val) + chunk0 + c);
+                    src[j] = __ldcg(p.cand_src + chunk0 + c);
                     key[j][0] = float_key_fast(v4.x); key[j][1] = float_key_fast(v4.y);
                     key[j][2] = float_key_fast(v4.z); key[j][3] = float_key_fast(v4.w);
                 } else {
@@ -537,7 +566,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                         while (ovf_mask && n_list >= 0) {
                             const int cc = j * 32 + __ffs(ovf_mask) - 1;
                             ovf_mask &= ovf_mask - 1u;
-                            const uint32_t k32 = float_key(__ldg(zr + cc * 32 + lane));
+                            const uint32_t k32 = float_key(__ldcg(zr + cc * 32 + lane));
                             const bool pred = k32 >= tE;
                             const uint32_t b = __ballot_sync(0xffffffffu, pred);
                             if (n_list + __popc(b) > cap) { n_list = -1; break; }   // too many ties: full scan
@@ -589,7 +618,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                 } else {
                     const uint32_t thr_full = warp_radix_select(GlobalKeys{zr}, V, tk, hist, lane);
                     for (int v = lane; v < V; v += 32) {
-                        const float zv = __ldg(zr + v);
+                        const float zv = __ldcg(zr + v);
                         if (float_key(zv) >= thr_full)
                             best_update(best, greedy ? zv + 0.0f : zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
                     }
@@ -600,7 +629,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
             uint32_t thr_full = 0u;
             if (filter) thr_full = warp_radix_select(GlobalKeys{zr}, V, tk, hist, lane);
             for (int v = lane; v < V; v += 32) {
-                const float zv = __ldg(zr + v);
+                const float zv = __ldcg(zr + v);
                 if (float_key(zv) >= thr_full)
                     best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
             }
@@ -608,12 +637,20 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         best = warp_argmax(best);
         token = best.v;
     }
-    if (lane == 0) {
+    if (valid && lane == 0) {
         p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
         if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
         if (p.delayed) {
             const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
             p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
+        }
+    }
+    if (p.ready) {
+        // the last CTA to finish re-arms the counters for the next step's K1 (which starts after this grid)
+        __syncthreads();
+        if (threadIdx.x == 0 && atomicAdd(p.done, 1) == static_cast<int>(gridDim.x) - 1) {
+            for (int g = 0; g < p.S * p.num_row_blocks; ++g) p.ready[g] = 0;
+            *p.done = 0;
         }
     }
 }

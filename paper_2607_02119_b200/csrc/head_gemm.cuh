@@ -25,6 +25,15 @@
 //               2 accumulator stages in TMEM so the epilogue of tile t overlaps the mainloop of t+1
 //   warps 2-9   epilogue, two warps per TMEM lane quarter (alternate 64-column slab pairs):
 //               tcgen05.ld -> merge -> x 1/temp -> z spill (fp32) -> per-chunk top-4 candidates
+//
+// Register budget: the register file is split over the SM's four sub-partitions (16 K registers
+// each) and the ten warps land 3/3/2/2 on them.  At 168 registers per thread a three-warp
+// sub-partition is full (16128 of 16384), so NO warp of any other grid can become resident on the
+// SM (measured: even a 32-thread kernel waits for this one to exit; setmaxnreg.dec does not help,
+// it returns registers to the CTA's own pool only).  Capped at 152, every sub-partition keeps
+// >= 1792 registers free = one 48..56-register warp of the finalize kernel (K2), which is what
+// lets K2's CTAs sit beside this kernel and sample finished (stream, row block) groups while
+// the GEMM is still running.
 #pragma once
 #include "ptx_sm100.cuh"
 
@@ -34,7 +43,9 @@ constexpr int kBM = 128;        // vocabulary rows per CTA tile (UMMA M, or half
 constexpr int kBK = 64;         // K elements per stage (128 B = swizzle span)
 constexpr int kMaxBN = 256;     // batch rows per tile (UMMA N)
 constexpr int kEpiWarps = 8;
-constexpr int kGemmThreads = 64 + 32 * kEpiWarps;
+constexpr int kCtrlWarps = 2;     // TMA producer, MMA issuer
+constexpr int kGemmMaxRegs = 152; // see "Register budget" above
+constexpr int kGemmThreads = 32 * (kCtrlWarps + kEpiWarps);
 constexpr int kMaxStages = 8;
 constexpr int kTmemCols = 512;
 constexpr int kCoefSlots = 512; // two-row slots whose coefficients fit the shared-memory table (R <= 1024)
@@ -62,6 +73,8 @@ struct GemmParams {
     float* cand_val;     // nullable [R][NT/32][4]: four z of every 32-token chunk, descending (see below)
     uint32_t* cand_src;  // nullable [R][NT/32]: their token offsets inside the chunk, 8 bits each
     int* err;            // sticky error word {code | row << 8}
+    int* ready;          // nullable [S][num_row_blocks]: epilogue-warp arrivals per (stream, row block), see K2
+    int V;               // tokens per stream (ready != nullptr requires V % kBM == 0)
     uint64_t policy_w, policy_h;
 };
 
@@ -145,7 +158,7 @@ __device__ __forceinline__ void chunk_top4(const float* col, float (&val)[4], ui
 }
 
 template <bool kTap, bool kCand, bool kPair>
-__global__ void __launch_bounds__(kGemmThreads, 1)
+__global__ void __maxnreg__(kGemmMaxRegs)
 cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
                        const GemmParams p) {
     extern __shared__ uint8_t smem_raw[];
@@ -200,6 +213,10 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
     if (kPair) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
+    // Every CTA is resident from here on: let the finalize grid (K2, launched with programmatic
+    // stream serialization) be scheduled beside this one.  It consumes finished (stream, row
+    // block) groups through p.ready while the GEMM is still running.
+    pdl_launch_dependents();
 
     if (warp == 0) {
         // ================= TMA producer (every CTA) =================
@@ -272,7 +289,7 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
         }
     } else {
         // ================= epilogue (warps 2..9, every CTA) =================
-        const int ew = warp - 2;
+        const int ew = warp - kCtrlWarps;
         const int quarter = warp & 3;             // TMEM lane quarter this warp may read
         const int half = ew >> 2;                 // which slab pairs (alternating) this warp takes
         const int et = ew * 32 + lane;            // 0..255 among epilogue threads
@@ -393,6 +410,11 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
                         __syncwarp();
                     }
                 }
+            }
+            if (p.ready && vt * kBM < p.NT) {
+                // this warp's z / candidate stores of the tile are issued: publish them (release) to K2
+                __syncwarp();
+                if (lane == 0) red_release_gpu_add(p.ready + ((vt * kBM) / p.V) * p.num_row_blocks + rb, 1);
             }
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }

@@ -301,3 +301,45 @@ def test_errors_are_reported_not_fatal(dev):
     # the context still works after errors
     dw.pair_map = wl.pair_map.to(dev)
     compare_step(dw, 3, None, ParityStats())
+
+
+def test_overlapped_finalize_equals_serial_finalize(dev):
+    """K2 launched as a programmatic dependent of K1 (consuming finished (stream, row block) groups
+    through the ready counters) must sample exactly what the strictly
+    serial launch samples; many consecutive steps also exercise the counter re-arm, a multi-wave
+    GEMM (row_tile 64 -> several row blocks) and CUDA-graph replay of the programmatic edge."""
+    wl = workloads.make_config(2)
+    ov = DeviceWorkload(wl, dev)
+    ov64 = DeviceWorkload(wl, dev, row_tile=64)
+    ser = DeviceWorkload(wl, dev, no_overlap=True)
+    for t in (0, 3, 8, 9, 10, 100, 250, 255):
+        for dw in (ov, ov64, ser):
+            dw.step(t)
+        torch.cuda.synchronize()
+        assert torch.equal(ov.tokens, ser.tokens) and torch.equal(ov64.tokens, ser.tokens)
+    assert torch.equal(ov.delayed, ser.delayed)
+    assert ov.ctx.info()["overlap"] == 1 and ser.ctx.info()["overlap"] == 0
+    waited, sampled = ov.ctx.overlap_stats()
+    assert sampled > 0 and ser.ctx.overlap_stats() == (0, 0)
+    # graph replay of the programmatic edge: the captured pair of steps, replayed, equals eager
+    steps = {t: wl.step(t).to(dev) for t in (20, 21)}
+    run = lambda t: ov.ctx.step(ov.hidden(t), ov.pair_map, ov.w, ov.temp, ov.top_k, wl.seed, steps[t], ov.tokens,
+                                req_id=ov.req_id, n_frames=ov.n_frames, delayed=ov.delayed)
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        run(20)
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g, stream=s):
+        run(20)
+        run(21)
+    ser.step(21)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        ov.tokens.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(ov.tokens, ser.tokens)
+    ov.check_no_device_error()
