@@ -57,10 +57,12 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
 
 #define CFGMS_CFG_SINGLE_CTA 4u  /* tuning/debug: never pair CTAs on one M = 256 MMA                */
 #define CFGMS_CFG_CTA_PAIR 8u    /* tuning/debug: always run the head GEMM on CTA pairs (cta_group::2) */
-#define CFGMS_CFG_NO_OVERLAP 16u /* tuning/debug: launch the finalize kernel strictly after the head
-                                    GEMM.  Default: it is launched as a programmatic dependent of the
-                                    GEMM and consumes finished (stream, row block) groups while the
-                                    GEMM is still running (candidate path with V % 128 == 0)        */
+#define CFGMS_CFG_NO_OVERLAP 16u /* tuning/debug: always launch the finalize kernel strictly after the
+                                    head GEMM.  Default: when the GEMM runs several waves of tiles, the
+                                    finalize kernel is launched as its programmatic dependent and samples
+                                    finished (stream, row block) groups while the GEMM is still running
+                                    (candidate path with V % 128 == 0)                                 */
+#define CFGMS_CFG_OVERLAP 32u    /* tuning/debug: overlap whenever eligible, even for a one-wave GEMM   */
 
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
@@ -180,12 +182,12 @@ int cfgms_profile_read(cfgms_ctx* ctx, double* gemm_ms, double* finalize_ms, int
 
 /*
  * Evidence that the finalize kernel really runs beside the head GEMM (cfgms_info.overlap = 1):
- * *cells_sampled = (request, stream) cells sampled on the overlapped path since the last call,
- * *cells_waited = how many of them reached their readiness check before the head GEMM had
- * finished their (stream, row block) group, i.e. while the GEMM was still running.  Both are 0
- * when the overlap is off.  One small D2H copy (synchronises the device); resets the counters.
+ * *cells_waited = (request, stream) cells that reached their readiness check before the head
+ * GEMM had finished their (stream, row block) group, i.e. while the GEMM was still running, since
+ * the last call.  0 when the overlap is off.  One small D2H copy (synchronises the device);
+ * resets the counter.
  */
-int cfgms_overlap_stats(cfgms_ctx* ctx, int64_t* cells_waited, int64_t* cells_sampled);
+int cfgms_overlap_stats(cfgms_ctx* ctx, int64_t* cells_waited);
 
 const char* cfgms_strerror(int status);
 /* Library build string: version, arch, compile flags. */

@@ -18,6 +18,7 @@ CFGMS_CFG_NO_CANDIDATES = 2
 CFGMS_CFG_SINGLE_CTA = 4
 CFGMS_CFG_CTA_PAIR = 8
 CFGMS_CFG_NO_OVERLAP = 16
+CFGMS_CFG_OVERLAP = 32
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
           5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
@@ -87,7 +88,7 @@ def _lib():
         L.cfgms_profile_read.restype = C.c_int
         L.cfgms_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cfgms_overlap_stats.restype = C.c_int
-        L.cfgms_overlap_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.cfgms_overlap_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
         L.cfgms_strerror.restype = C.c_char_p
         L.cfgms_strerror.argtypes = [C.c_int]
         L.cfgms_version.restype = C.c_char_p
@@ -133,7 +134,8 @@ class Context:
 
     def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
-                 cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0):
+                 cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0,
+                 force_overlap: bool = False):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -153,6 +155,8 @@ class Context:
             cfg.flags |= CFGMS_CFG_CTA_PAIR if cta_pair else CFGMS_CFG_SINGLE_CTA
         if no_overlap:             # tuning: finalize strictly after the head GEMM
             cfg.flags |= CFGMS_CFG_NO_OVERLAP
+        elif force_overlap:        # tuning: overlap even for a one-wave GEMM
+            cfg.flags |= CFGMS_CFG_OVERLAP
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):
@@ -260,14 +264,14 @@ class Context:
             raise CfgmsError(rc, "cfgms_profile_read")
         return float(g.value), float(f.value), int(n.value)
 
-    def overlap_stats(self):
-        """-> (cells that reached their readiness check while the head GEMM was still producing their
-        group, cells sampled on the overlapped path) since the last call; synchronises."""
-        w, n = C.c_int64(), C.c_int64()
-        rc = _lib().cfgms_overlap_stats(self._h, C.byref(w), C.byref(n))
+    def overlap_stats(self) -> int:
+        """-> cells that reached their readiness check while the head GEMM was still producing their
+        group, since the last call (evidence of the K1/K2 overlap); synchronises."""
+        w = C.c_int64()
+        rc = _lib().cfgms_overlap_stats(self._h, C.byref(w))
         if rc != 0:
             raise CfgmsError(rc, "cfgms_overlap_stats")
-        return int(w.value), int(n.value)
+        return int(w.value)
 
     def info(self) -> dict:
         inf = cfgms_info()

@@ -24,6 +24,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 constexpr int kProfMax = 4096;
+constexpr int kOverlapMinWaves = 3;
 
 struct HostStage {  // device staging for the *_host entry points
     void* hidden = nullptr;
@@ -52,7 +53,8 @@ struct cfgms_ctx {
     int* err = nullptr;               // device: sticky {code | row << 8}
     int* ready = nullptr;             // device: [S][row blocks] K1 -> K2 tile arrivals, then one `done` counter
     int ready_words = 0;
-    bool overlap = false;             // K2 as a programmatic dependent of K1 (candidate path, V % 128 == 0)
+    bool overlap = false;             // K2 may run as a programmatic dependent of K1 (candidate path, V % 128 == 0)
+    int overlap_mode = 0;             // 0 = when the GEMM has >= kOverlapMinWaves waves, 1 = never, 2 = whenever eligible
     EncodeTiledFn encode = nullptr;
     CUtensorMap tmap_w;
     CUtensorMap tmap_h;
@@ -201,9 +203,10 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
         return rc;
     }
     cudaMemset(c->err, 0, 2 * sizeof(int));
-    c->overlap = c->use_cand && (V % kBM) == 0 && !(cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP));
+    c->overlap_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_OVERLAP)) ? 2 : 0;
+    c->overlap = c->use_cand && (V % kBM) == 0 && c->overlap_mode != 1;
     if (c->overlap) {
-        c->ready_words = ((S * ((c->max_rows + 63) / 64) + 1 + 1) & ~1) + 4;   // counters | done | pad | stats (2 x u64)
+        c->ready_words = ((S * ((c->max_rows + 63) / 64) + 1 + 1) & ~1) + 32;   // counters | done | pad | stats (16 x u64)
         if ((rc = dev_alloc(&c->ready, static_cast<size_t>(c->ready_words))) != CFGMS_OK) {
             cfgms_destroy(c);
             return rc;
@@ -239,6 +242,10 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, false, true>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<false, true, true>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, true, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<false, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<true, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<false, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<true, true>));
     if (!attr_ok ||
         cudaFuncSetAttribute(cfgms_finalize_cand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
         cfgms_destroy(c);
@@ -320,15 +327,20 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp;
     gp.bias = c->bias; gp.z = c->z; gp.tap = a->logits_out; gp.err = c->err;
     gp.cand_val = c->cand_val; gp.cand_src = c->cand_src;
-    gp.ready = c->overlap ? c->ready : nullptr;
+    const int workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
+    const bool prof = c->prof_on && c->prof_n < kProfMax;
+    // Overlap K2 with K1 only where finished groups appear long before the GEMM ends (several waves of
+    // tiles): a one- or two-wave GEMM has nothing to hide behind, and the lean register budget and
+    // the polling finalize warps then cost more than the early launch saves (measured).
+    const bool overlap = c->overlap && !prof &&
+                         (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
+    gp.ready = overlap ? c->ready : nullptr;
     gp.V = c->V;
     // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;
-    const int workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
     const int grid = pair ? 2 * workers : workers;
     const size_t smem = GemmSmemLayout::total(b_rows, stages);
-    const bool prof = c->prof_on && c->prof_n < kProfMax;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
     {
         using KernelFn = void (*)(const CUtensorMap, const CUtensorMap, const GemmParams);
@@ -337,7 +349,10 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
             cfgms_head_gemm_kernel<false, true, false>,  cfgms_head_gemm_kernel<true, true, false>,
             cfgms_head_gemm_kernel<false, false, true>,  cfgms_head_gemm_kernel<true, false, true>,
             cfgms_head_gemm_kernel<false, true, true>,   cfgms_head_gemm_kernel<true, true, true>};
-        const KernelFn fn = table[(a->logits_out ? 1 : 0) | (c->use_cand ? 2 : 0) | (pair ? 4 : 0)];
+        static const KernelFn lean[4] = {cfgms_head_gemm_lean_kernel<false, false>, cfgms_head_gemm_lean_kernel<true, false>,
+                                         cfgms_head_gemm_lean_kernel<false, true>, cfgms_head_gemm_lean_kernel<true, true>};
+        const KernelFn fn = overlap ? lean[(a->logits_out ? 1 : 0) | (pair ? 2 : 0)]
+                                    : table[(a->logits_out ? 1 : 0) | (c->use_cand ? 2 : 0) | (pair ? 4 : 0)];
         cudaLaunchConfig_t lc{};
         lc.gridDim = dim3(static_cast<unsigned>(grid));
         lc.blockDim = dim3(kGemmThreads);
@@ -365,8 +380,8 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
     fp.cand_val = c->cand_val; fp.cand_src = c->cand_src;
     fp.ready = gp.ready;
-    fp.done = c->overlap ? c->ready + (c->ready_words - 5) : nullptr;
-    fp.stats = c->overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 4)) : nullptr;
+    fp.done = overlap ? c->ready + (c->ready_words - 33) : nullptr;
+    fp.stats = overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 32)) : nullptr;
     fp.err = c->err;
     fp.BN = BN; fp.num_row_blocks = nrb;
     fp.ready_target = (c->V / kBM) * kEpiWarps;   // every epilogue warp of every vocabulary tile of the stream
@@ -389,7 +404,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         lc.attrs = attr;
-        lc.numAttrs = (c->overlap && !prof) ? 1 : 0;
+        lc.numAttrs = overlap ? 1 : 0;
         if (cudaLaunchKernelEx(&lc, ffn, fp) != cudaSuccess) return CFGMS_ERR_CUDA;
     } else {
         const dim3 fgrid(c->S, a->R);
@@ -406,7 +421,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
     c->info.cta_pair = pair ? 1 : 0;
-    c->info.overlap = (c->overlap && !prof) ? 1 : 0;
+    c->info.overlap = overlap ? 1 : 0;
     c->info.launches_last_step = launches;
     c->info.launches_total += launches;
     c->info.h2d_bytes_last_step = 0; c->info.d2h_bytes_last_step = 0;
@@ -508,7 +523,7 @@ int cfgms_last_device_error(cfgms_ctx* c, int32_t* row_out) {
     if (word[0] == 0) return CFGMS_OK;
     if (row_out) *row_out = word[0] >> 8;
     cudaMemset(c->err, 0, sizeof(word));
-    if (c->ready) cudaMemset(c->ready, 0, static_cast<size_t>(c->ready_words - 4) * sizeof(int));   // a failed step may leave them armed
+    if (c->ready) cudaMemset(c->ready, 0, static_cast<size_t>(c->ready_words - 32) * sizeof(int));   // a failed step may leave them armed
     return word[0] & 0xff;
 }
 
@@ -542,16 +557,15 @@ int cfgms_profile_read(cfgms_ctx* c, double* gemm_ms, double* finalize_ms, int64
     return CFGMS_OK;
 }
 
-int cfgms_overlap_stats(cfgms_ctx* c, int64_t* cells_waited, int64_t* cells_sampled) {
-    if (!c || !cells_waited || !cells_sampled) return CFGMS_ERR_ARG;
-    *cells_waited = *cells_sampled = 0;
+int cfgms_overlap_stats(cfgms_ctx* c, int64_t* cells_waited) {
+    if (!c || !cells_waited) return CFGMS_ERR_ARG;
+    *cells_waited = 0;
     if (!c->ready) return CFGMS_OK;
-    unsigned long long w[2] = {0, 0};
-    int* st = c->ready + (c->ready_words - 4);
+    unsigned long long w[16];
+    int* st = c->ready + (c->ready_words - 32);
     if (cudaMemcpy(w, st, sizeof(w), cudaMemcpyDeviceToHost) != cudaSuccess) return CFGMS_ERR_CUDA;
     if (cudaMemset(st, 0, sizeof(w)) != cudaSuccess) return CFGMS_ERR_CUDA;
-    *cells_waited = static_cast<int64_t>(w[0]);
-    *cells_sampled = static_cast<int64_t>(w[1]);
+    for (int j = 0; j < 16; ++j) *cells_waited += static_cast<int64_t>(w[j]);
     return CFGMS_OK;
 }
 

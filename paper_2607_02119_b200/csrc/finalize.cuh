@@ -44,7 +44,7 @@ struct FinalizeParams {
     // (stream, row block) in ready[]; a cell is consumed once its group reached ready_target.
     int* ready;               // nullable [S][num_row_blocks]
     int* done;                // CTAs of this grid that finished; the last one clears ready[] for the next step
-    unsigned long long* stats;// {cells that arrived before their group was complete, cells sampled}
+    unsigned long long* stats;// [16] cells that arrived before their group was complete (summed on the host)
     int* err;                 // sticky error word
     int BN, num_row_blocks, ready_target;
 };
@@ -414,9 +414,8 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
             // wait until K1 has written every tile of this (stream, row block): acquire pairs with
             // the epilogue warps' red.release; bounded so a pipeline bug fails loudly
             const int* flag = p.ready + i * p.num_row_blocks + r / p.BN;
-            if (lane == 0) atomicAdd(p.stats + 1, 1ull);
             if (lane == 0 && ld_acquire_gpu(flag) < p.ready_target) {
-                atomicAdd(p.stats, 1ull);
+                atomicAdd(p.stats + (blockIdx.x & 15), 1ull);   // evidence counter, spread over 16 words
                 const uint64_t t0 = global_timer_ns();
                 while (ld_acquire_gpu(flag) < p.ready_target) {
                     __nanosleep(200);

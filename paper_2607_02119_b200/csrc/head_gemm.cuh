@@ -158,9 +158,7 @@ __device__ __forceinline__ void chunk_top4(const float* col, float (&val)[4], ui
 }
 
 template <bool kTap, bool kCand, bool kPair>
-__global__ void __maxnreg__(kGemmMaxRegs)
-cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
-                       const GemmParams p) {
+__device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const CUtensorMap& tmap_h, const GemmParams& p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const int stages = p.stages;
@@ -426,6 +424,23 @@ cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_
         tc_fence_after();
         if (kPair) tmem_dealloc_pair(tmem_base, kTmemCols); else tmem_dealloc(tmem_base, kTmemCols);
     }
+}
+
+// Full register budget (168): the fastest GEMM, but nothing else fits on its SMs while it runs.
+template <bool kTap, bool kCand, bool kPair>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
+                       const GemmParams p) {
+    head_gemm_body<kTap, kCand, kPair>(tmap_w, tmap_h, p);
+}
+
+// Lean register budget (see "Register budget" above): leaves room for the finalize kernel's CTAs on
+// the same SMs; used when K2 is launched as a programmatic dependent of a multi-wave GEMM.
+template <bool kTap, bool kPair>
+__global__ void __maxnreg__(kGemmMaxRegs)
+cfgms_head_gemm_lean_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
+                            const GemmParams p) {
+    head_gemm_body<kTap, true, kPair>(tmap_w, tmap_h, p);
 }
 
 }  // namespace cfgms
