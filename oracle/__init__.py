@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "cfgms_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-FLAG_INACTIVE, FLAG_GREEDY, FLAG_CLOSE, FLAG_BOUNDARY = 1, 2, 4, 8
+FLAG_INACTIVE, FLAG_GREEDY, FLAG_CLOSE, FLAG_BOUNDARY, FLAG_FORCED = 1, 2, 4, 8, 16
 TOL = 2e-2  # north_star's margin below which a tie is "close" (counted, not failed)
 
 
@@ -52,6 +52,12 @@ def lib():
         L.oracle_step.argtypes = ([C.c_void_p] * 3 + [C.c_int32] * 4 + [C.c_void_p] * 4 + [C.c_uint64]
                                   + [C.c_void_p] * 3 + [C.c_int32, C.c_double, C.c_void_p, C.c_int64]
                                   + [C.c_void_p] * 6 + [C.c_int32])
+        L.oracle_step_ex.restype = C.c_int
+        L.oracle_step_ex.argtypes = L.oracle_step.argtypes + [C.c_void_p, C.c_void_p]
+        L.oracle_emit_frame.restype = C.c_int32
+        L.oracle_emit_frame.argtypes = [C.c_void_p] + [C.c_int32] * 5 + [C.c_void_p]
+        L.oracle_feedback.restype = None
+        L.oracle_feedback.argtypes = [C.c_void_p, C.c_void_p] + [C.c_int32] * 4 + [C.c_void_p]
         L.oracle_logits_row.restype = None
         L.oracle_logits_row.argtypes = [C.c_void_p] * 3 + [C.c_int32] * 5 + [C.c_void_p]
         L.oracle_cfg_merge.restype = None
@@ -172,7 +178,7 @@ class StepResult:
 def step(heads, embeds, hidden, pair_map, w, temp, top_k, seed: int, step_, req_id=None,
          n_frames=None, pad_token: Optional[int] = None, cells=None, want_merged: bool = False,
          tokens_out: Optional[np.ndarray] = None, delayed: Optional[np.ndarray] = None,
-         tol: float = TOL, hidden_is_f32: bool = False) -> StepResult:
+         tol: float = TOL, hidden_is_f32: bool = False, logit_bias=None, force_token=None) -> StepResult:
     """One decode step (O1-O10).  `hidden` is bf16 (torch) or, with hidden_is_f32, fp32 that is
     first rounded to bf16 (C18).  `cells` = None (all) or int array [n][2] of (row, stream)."""
     h = _arr(heads, np.uint16)
@@ -208,10 +214,16 @@ def step(heads, embeds, hidden, pair_map, w, temp, top_k, seed: int, step_, req_
         T_cap = delayed.shape[1]
     if tokens_out is not None:
         assert tokens_out.dtype == np.int32 and tokens_out.flags.c_contiguous
-    rc = lib().oracle_step(_p(h), _p(e), _p(x), R, S, d, V, _p(pm), _p(ww), _p(tt), _p(kk),
-                           C.c_uint64(seed), _p(st), _p(rid), _p(nf), pad, C.c_double(tol),
-                           _p(cl), C.c_int64(n), _p(res.tok), _p(res.margin), _p(res.flags),
-                           _p(res.merged), _p(tokens_out), _p(delayed), T_cap)
+    lb = _arr(logit_bias, np.float64)     # widening W2: [S][V] additive bias (-inf masks a token)
+    ft = _arr(force_token, np.int32)      # widening W2: [R][S], >= 0 forces the cell's token
+    if lb is not None:
+        assert lb.shape == (S, V)
+    if ft is not None:
+        assert ft.shape == (R, S)
+    rc = lib().oracle_step_ex(_p(h), _p(e), _p(x), R, S, d, V, _p(pm), _p(ww), _p(tt), _p(kk),
+                              C.c_uint64(seed), _p(st), _p(rid), _p(nf), pad, C.c_double(tol),
+                              _p(cl), C.c_int64(n), _p(res.tok), _p(res.margin), _p(res.flags),
+                              _p(res.merged), _p(tokens_out), _p(delayed), T_cap, _p(lb), _p(ft))
     if rc != 0:
         raise ValueError(f"oracle_step failed with code {rc}")
     return res
@@ -242,3 +254,25 @@ def interleave(grid: np.ndarray, pad: int) -> np.ndarray:
     if rc != 0:
         raise ValueError(f"oracle_interleave failed with code {rc}")
     return dl
+
+
+def emit_frame(ring: np.ndarray, tau: int, n_frames: int, pad: int):
+    """Widening W1.  ring: int32 [T_cap][S] of ONE request (ring[t % T_cap][i] = token of stream i
+    at step t).  -> (frame index or -1, frame int32 [S])."""
+    rg = np.ascontiguousarray(ring, dtype=np.int32)
+    T_cap, S = rg.shape
+    frame = np.empty(S, dtype=np.int32)
+    f = lib().oracle_emit_frame(_p(rg), T_cap, S, int(tau), int(n_frames), int(pad), _p(frame))
+    return int(f), frame
+
+
+def feedback(tokens, emb) -> np.ndarray:
+    """Widening W3.  tokens int32 [R][S], emb bf16 [S][V_e][d] -> float64 [R][d] (exact sums)."""
+    tk = _arr(tokens, np.int32)
+    eb = _arr(emb, np.uint16)
+    R, S = tk.shape
+    S2, V_e, d = eb.shape
+    assert S == S2
+    x = np.empty((R, d), dtype=np.float64)
+    lib().oracle_feedback(_p(tk), _p(eb), R, S, V_e, d, _p(x))
+    return x

@@ -30,6 +30,15 @@
  *   O9 tokens_out[cond] = tokens_out[uncond] = token
  *      delayed[c][tau mod T_cap][i] = token  (PAD when inactive)
  *   de-interleave: G[q][f][i] = D[q][f + i][i], F = T - S + 1
+ * Widenings, each pinned in tests/test_oracle_widen.py:
+ *   W1 oracle_emit_frame   streaming frame emission from the delay ring
+ *      pin: emission over all steps == oracle_deinterleave of the full delayed matrix, for every
+ *      ring depth >= S; hand-written 3-stream example
+ *   W2 oracle_step_ex      static logit bias (vocabulary mask) + forced tokens
+ *      pin: zero bias / no forcing == oracle_step bit-exactly; -inf mask == sampling on the
+ *      reduced vocabulary (chi-square vs softmax over the unmasked tokens); forced cells verbatim
+ *   W3 oracle_feedback     sum of the sampled tokens' stream embeddings
+ *      pin: torch fp64 gather-sum; one stream == row copy; out-of-range ids contribute zero
  */
 #include <math.h>
 #include <stdint.h>
@@ -48,6 +57,7 @@
 #define ORC_GREEDY 2     /* took the explicit argmax branch O6                            */
 #define ORC_CLOSE 4      /* best-minus-second perturbed score <= tol (north_star's rule)  */
 #define ORC_BOUNDARY 8   /* outcome could change if z moved by < tol at the top-k edge    */
+#define ORC_FORCED 16    /* token given by force_token, nothing sampled                   */
 
 int oracle_num_threads(void) {
 #ifdef _OPENMP
@@ -222,14 +232,23 @@ int oracle_check_pair_map(const int32_t* pair_map, int32_t R) {
  * merged_out != NULL merged_out[j][V] (pre-temperature merged logits, zeros for PAD cells).
  * tokens_out [R][S] and delayed [R][T_cap][S] (both nullable) receive O9's writes for the
  * evaluated cells only; other entries are left untouched. */
-int oracle_step(const uint16_t* heads, const uint16_t* embeds, const uint16_t* hidden,
-                int32_t R, int32_t S, int32_t d, int32_t V,
-                const int32_t* pair_map, const float* w, const float* temp, const int32_t* top_k,
-                uint64_t seed, const int32_t* step, const uint32_t* req_id, const int32_t* n_frames,
-                int32_t pad_token, double tol,
-                const int32_t* cells, int64_t n_cells,
-                int32_t* tok_out, double* margin_out, int32_t* flags_out, double* merged_out,
-                int32_t* tokens_out, int32_t* delayed, int32_t T_cap) {
+/* Widening W2 (the hooks through which the phase state machine of
+ * PAPER.md:70-76 acts on the audio head):
+ *   logit_bias  nullable double [S][V]: merged logits become M + bias[i][v] BEFORE the
+ *               temperature ("dynamic vocabulary masking": -inf removes a token);
+ *   force_token nullable int32 [R][S], read at the request-owning row: a value >= 0 is emitted
+ *               as the cell's token without sampling (a deterministic bridging token of the
+ *               transition phase, or the padding of a text-phase row); < 0 = sample normally.
+ *               It is only consulted for ACTIVE cells: the delay pattern's PAD wins. */
+int oracle_step_ex(const uint16_t* heads, const uint16_t* embeds, const uint16_t* hidden,
+                   int32_t R, int32_t S, int32_t d, int32_t V,
+                   const int32_t* pair_map, const float* w, const float* temp, const int32_t* top_k,
+                   uint64_t seed, const int32_t* step, const uint32_t* req_id, const int32_t* n_frames,
+                   int32_t pad_token, double tol,
+                   const int32_t* cells, int64_t n_cells,
+                   int32_t* tok_out, double* margin_out, int32_t* flags_out, double* merged_out,
+                   int32_t* tokens_out, int32_t* delayed, int32_t T_cap,
+                   const double* logit_bias, const int32_t* force_token) {
     if (R <= 0 || S <= 0 || d <= 0 || V <= 0) return ORACLE_ERR_ARG;
     int rc = oracle_check_pair_map(pair_map, R);
     if (rc != ORACLE_OK) return rc;
@@ -267,6 +286,10 @@ int oracle_step(const uint16_t* heads, const uint16_t* embeds, const uint16_t* h
             tok = pad_token;
             flags = ORC_INACTIVE;
             if (merged_out) memset(merged_out + (size_t)j * V, 0, sizeof(double) * (size_t)V);
+        } else if (force_token && force_token[(size_t)c * S + i] >= 0) {
+            tok = force_token[(size_t)c * S + i];
+            flags = ORC_FORCED;
+            if (merged_out) memset(merged_out + (size_t)j * V, 0, sizeof(double) * (size_t)V);
         } else {
             double* Lc = (double*)malloc(sizeof(double) * (size_t)V * 3);
             double* Lu = Lc + V;
@@ -278,6 +301,8 @@ int oracle_step(const uint16_t* heads, const uint16_t* embeds, const uint16_t* h
             } else {
                 memcpy(M, Lc, sizeof(double) * (size_t)V);
             }
+            if (logit_bias)
+                for (int32_t v = 0; v < V; ++v) M[v] += logit_bias[(size_t)i * V + v];
             tok = oracle_sample_cell(M, V, temp[c], top_k[c], seed, rid, tau, i, tol,
                                      &margin, &flags, NULL);                         /* O6-O8 */
             if (merged_out) memcpy(merged_out + (size_t)j * V, M, sizeof(double) * (size_t)V);
@@ -297,6 +322,19 @@ int oracle_step(const uint16_t* heads, const uint16_t* embeds, const uint16_t* h
     }
     free(all_cells);
     return ORACLE_OK;
+}
+
+int oracle_step(const uint16_t* heads, const uint16_t* embeds, const uint16_t* hidden,
+                int32_t R, int32_t S, int32_t d, int32_t V,
+                const int32_t* pair_map, const float* w, const float* temp, const int32_t* top_k,
+                uint64_t seed, const int32_t* step, const uint32_t* req_id, const int32_t* n_frames,
+                int32_t pad_token, double tol,
+                const int32_t* cells, int64_t n_cells,
+                int32_t* tok_out, double* margin_out, int32_t* flags_out, double* merged_out,
+                int32_t* tokens_out, int32_t* delayed, int32_t T_cap) {
+    return oracle_step_ex(heads, embeds, hidden, R, S, d, V, pair_map, w, temp, top_k, seed, step, req_id,
+                          n_frames, pad_token, tol, cells, n_cells, tok_out, margin_out, flags_out,
+                          merged_out, tokens_out, delayed, T_cap, NULL, NULL);
 }
 
 /* ---- delay pattern ------------------------------------------------------------------------ */
@@ -323,6 +361,41 @@ int oracle_interleave(const int32_t* grid, int32_t n, int32_t F, int32_t S, int3
                     (f >= 0 && f < F) ? grid[((size_t)q * F + f) * S + i] : pad;
             }
     return ORACLE_OK;
+}
+
+/* Widening W1 — streaming finished-frame emission ("fusing waveform synthesis
+ * directly into the serving path", Fig. 2 left).  After step tau of a
+ * request whose delayed tokens live in a ring of depth T_cap >= S (ring[t mod T_cap][i] = token
+ * of stream i sampled at step t), frame f = tau - S + 1 is complete iff 0 <= f < F:
+ *     frame[i] = ring[(f + i) mod T_cap][i]        (= D[f + i][i], the de-interleave rule)
+ * Returns f, or -1 when no frame completes at this step (frame[] is then filled with pad). */
+int32_t oracle_emit_frame(const int32_t* ring, int32_t T_cap, int32_t S, int32_t tau, int32_t F,
+                          int32_t pad, int32_t* frame) {
+    int32_t f = tau - S + 1;
+    if (f < 0 || (F >= 0 && f >= F) || T_cap < S) {
+        for (int32_t i = 0; i < S; ++i) frame[i] = pad;
+        return -1;
+    }
+    for (int32_t i = 0; i < S; ++i) frame[i] = ring[(size_t)((f + i) % T_cap) * S + i];
+    return f;
+}
+
+/* Widening W3 — autoregressive feedback aggregation ("the input representation at
+ * each step aggregates the embeddings of these previously generated tokens"; reading C25: the
+ * aggregate is the SUM over the S streams of the stream's own embedding row of its token).
+ *     x[r][k] = sum_{i=0}^{S-1} Emb_i[tokens[r][i]][k]        i ascending, fp64
+ * emb: bf16 [S][V_e][d]; a token id outside [0, V_e) contributes nothing. */
+void oracle_feedback(const int32_t* tokens, const uint16_t* emb, int32_t R, int32_t S, int32_t V_e, int32_t d,
+                     double* x) {
+    for (int32_t r = 0; r < R; ++r)
+        for (int32_t k = 0; k < d; ++k) {
+            double acc = 0.0;
+            for (int32_t i = 0; i < S; ++i) {
+                int32_t t = tokens[(size_t)r * S + i];
+                if (t >= 0 && t < V_e) acc += bf16_to_double(emb[((size_t)i * V_e + t) * d + k]);
+            }
+            x[(size_t)r * d + k] = acc;
+        }
 }
 
 /* ---- test helper: empirical token frequencies of O6-O8 on fixed merged logits ------------- */
