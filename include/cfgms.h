@@ -116,6 +116,19 @@ typedef struct {
     int32_t T_cap;
     float* logits_out;        /* nullable DEBUG tap: merged pre-temperature logits fp32
                                  [R][S][V], valid at cond / unpaired rows                        */
+    /* --- widenings (all nullable; NULL leaves the step exactly as described above) --- */
+    const int32_t* force_token; /* [R][S], read at the cond / unpaired row: a value >= 0 is emitted
+                                 as that cell's token without sampling — the hook for the phase
+                                 state machine's deterministic bridging tokens and text-phase
+                                 padding; < 0 = sample.  Only consulted for cells
+                                 the delay pattern leaves active (PAD wins otherwise)            */
+    int32_t* frame_out;       /* [R][S] streaming frame emission: when frame
+                                 f = tau - S + 1 of the request completes at this step
+                                 (0 <= f < n_frames), frame_out[r][i] = delayed[r][(f+i) mod T_cap][i];
+                                 otherwise the row is filled with the pad token.  Needs `delayed`
+                                 with T_cap >= S (else CFGMS_ERR_ARG).  Companion rows: pad      */
+    int32_t* frame_index_out; /* [R] the frame index f emitted for the row, or -1 (also -1 at
+                                 companion rows, whose outputs stay hidden)         */
 } cfgms_step_args;
 
 /*
@@ -129,12 +142,34 @@ int cfgms_step(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stream);
 
 /*
  * cfgms_step_host — same step with HOST buffers: hidden, pair_map, w, temp, top_k, step,
- * req_id, n_frames and tokens_out are HOST pointers (pinned memory recommended); `delayed`
- * and `logits_out` stay DEVICE pointers (per-request state lives in HBM) or NULL.  Copies the
+ * req_id, n_frames, force_token, tokens_out, frame_out and frame_index_out are HOST pointers
+ * (pinned memory recommended); `delayed` and `logits_out` stay DEVICE pointers (per-request state lives in HBM) or NULL.  Copies the
  * inputs host->device, runs the step, copies tokens_out device->host and synchronises the
  * stream.  Bytes moved per call are reported by cfgms_get_info.
  */
 int cfgms_step_host(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stream);
+
+/*
+ * cfgms_set_logit_bias — dynamic vocabulary masking hook.  bias: DEVICE fp32
+ * [S][V] added to the merged logits of every request before the temperature (-inf removes a
+ * token from stream i's vocabulary), or NULL to clear it.  Folded into the library's own
+ * per-token bias once, on `cuda_stream`; costs nothing per step.  Not retained.
+ */
+int cfgms_set_logit_bias(cfgms_ctx* ctx, const float* bias, void* cuda_stream);
+
+/*
+ * cfgms_feedback — autoregressive feedback aggregation ("the input representation
+ * at each step aggregates the embeddings of these previously generated tokens"):
+ *     x_out[r][k] = bf16_rne( sum_{i < S} emb[i][tokens[r][i]][k] )     (fp32 sum, i ascending)
+ *   tokens : DEVICE int32 [R][S] (cfgms_step's tokens_out: a companion row carries its cond
+ *            row's tokens, so both get the same input row)
+ *   emb    : DEVICE bf16 [S][V_e][d] token-embedding tables, one per stream; a token id outside
+ *            [0, V_e) (e.g. a pad id with no embedding row) contributes nothing
+ *   x_out  : DEVICE bf16 [R][d]
+ * S and d are the context's.  Enqueues on `cuda_stream`; does not synchronise.  Errors: ARG.
+ */
+int cfgms_feedback(cfgms_ctx* ctx, const int32_t* tokens, const void* emb, int32_t V_e, int32_t R,
+                   void* x_out, void* cuda_stream);
 
 /*
  * cfgms_deinterleave — PAPER.md:56,68: grid[q][f][i] = delayed[q][f + i][i] for

@@ -25,7 +25,8 @@ STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR
 
 EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
-           "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats"]
+           "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats",
+           "cfgms_set_logit_bias", "cfgms_feedback"]
 
 
 class CfgmsError(RuntimeError):
@@ -44,7 +45,8 @@ class cfgms_step_args(C.Structure):
                 ("pair_map", C.c_void_p), ("w", C.c_void_p), ("temp", C.c_void_p), ("top_k", C.c_void_p),
                 ("seed", C.c_uint64), ("step", C.c_void_p), ("req_id", C.c_void_p), ("n_frames", C.c_void_p),
                 ("tokens_out", C.c_void_p), ("delayed", C.c_void_p), ("T_cap", C.c_int32),
-                ("logits_out", C.c_void_p)]
+                ("logits_out", C.c_void_p), ("force_token", C.c_void_p), ("frame_out", C.c_void_p),
+                ("frame_index_out", C.c_void_p)]
 
 
 class cfgms_info(C.Structure):
@@ -87,6 +89,10 @@ def _lib():
         L.cfgms_profile_enable.argtypes = [C.c_void_p, C.c_int]
         L.cfgms_profile_read.restype = C.c_int
         L.cfgms_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.cfgms_set_logit_bias.restype = C.c_int
+        L.cfgms_set_logit_bias.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.cfgms_feedback.restype = C.c_int
+        L.cfgms_feedback.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.cfgms_overlap_stats.restype = C.c_int
         L.cfgms_overlap_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
         L.cfgms_strerror.restype = C.c_char_p
@@ -179,7 +185,7 @@ class Context:
             pass
 
     def _args(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
-              logits_out, dev: str) -> cfgms_step_args:
+              logits_out, dev: str, force_token=None, frame_out=None, frame_index_out=None) -> cfgms_step_args:
         R = int(hidden.shape[0])
         _check(hidden, "hidden", (torch.bfloat16, torch.float32), dev, R * self.d)
         if hidden.dim() != 2 or hidden.shape[1] != self.d:
@@ -209,25 +215,56 @@ class Context:
             a.delayed = delayed.data_ptr()
             a.T_cap = int(delayed.shape[1])
         a.logits_out = _ptr(logits_out)
+        _check(force_token, "force_token", torch.int32, dev, R * self.S, optional=True)
+        _check(frame_out, "frame_out", torch.int32, dev, R * self.S, optional=True)
+        _check(frame_index_out, "frame_index_out", torch.int32, dev, R, optional=True)
+        a.force_token, a.frame_out, a.frame_index_out = _ptr(force_token), _ptr(frame_out), _ptr(frame_index_out)
         return a
 
     def step(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
-             delayed=None, logits_out=None, stream=None) -> None:
+             delayed=None, logits_out=None, stream=None, force_token=None, frame_out=None,
+             frame_index_out=None) -> None:
         """cfgms_step: device tensors, enqueue only."""
         a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
-                       logits_out, "cuda")
+                       logits_out, "cuda", force_token, frame_out, frame_index_out)
         rc = _lib().cfgms_step(self._h, C.byref(a), _stream_ptr(stream))
         if rc != 0:
             raise CfgmsError(rc, "cfgms_step")
 
     def step_host(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
-                  delayed=None, logits_out=None, stream=None) -> None:
+                  delayed=None, logits_out=None, stream=None, force_token=None, frame_out=None,
+                  frame_index_out=None) -> None:
         """cfgms_step_host: host tensors in, host tokens out; synchronises the stream."""
         a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
-                       logits_out, "cpu")
+                       logits_out, "cpu", force_token, frame_out, frame_index_out)
         rc = _lib().cfgms_step_host(self._h, C.byref(a), _stream_ptr(stream))
         if rc != 0:
             raise CfgmsError(rc, "cfgms_step_host")
+
+    def set_logit_bias(self, bias: Optional[torch.Tensor], stream=None) -> None:
+        """cfgms_set_logit_bias: fp32 [S][V] additive vocabulary mask / bias (cuda), or None to clear."""
+        _check(bias, "bias", torch.float32, "cuda", self.S * self.V, optional=True)
+        rc = _lib().cfgms_set_logit_bias(self._h, _ptr(bias), _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_set_logit_bias")
+
+    def feedback(self, tokens: torch.Tensor, emb: torch.Tensor, x_out: Optional[torch.Tensor] = None,
+                 stream=None) -> torch.Tensor:
+        """cfgms_feedback: tokens int32 [R][S], emb bf16 [S][V_e][d] -> x bf16 [R][d] (all cuda)."""
+        if tokens.dim() != 2 or tokens.shape[1] != self.S or emb.dim() != 3 or emb.shape[0] != self.S \
+                or emb.shape[2] != self.d:
+            raise ValueError("tokens must be [R][S] and emb [S][V_e][d]")
+        R, V_e = int(tokens.shape[0]), int(emb.shape[1])
+        _check(tokens, "tokens", torch.int32, "cuda", R * self.S)
+        _check(emb, "emb", torch.bfloat16, "cuda", self.S * V_e * self.d)
+        if x_out is None:
+            x_out = torch.empty((R, self.d), dtype=torch.bfloat16, device=tokens.device)
+        _check(x_out, "x_out", torch.bfloat16, "cuda", R * self.d)
+        rc = _lib().cfgms_feedback(self._h, tokens.data_ptr(), emb.data_ptr(), V_e, R, x_out.data_ptr(),
+                                   _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_feedback")
+        return x_out
 
     def deinterleave(self, delayed: torch.Tensor, grid_out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
         """cfgms_deinterleave(_host): [n][T][S] int32 -> [n][T-S+1][S]; host path if `delayed` is on the CPU."""

@@ -96,4 +96,78 @@ cfgms_cast_f32_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restri
         out[e] = __float2bfloat16_rn(in[e]);
 }
 
+// ---------------------------------------------------------------- K6 (PAPER.md:70-76 masking hook)
+// bias[n] = base[n] + user[n]: the caller's additive vocabulary mask / bias is folded into the
+// per-token bias the head GEMM's epilogue adds anyway.  user == nullptr restores the base.
+__global__ void __launch_bounds__(256)
+cfgms_bias_fold_kernel(const float* __restrict__ base, const float* __restrict__ user, float* __restrict__ bias, int n) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < n) bias[e] = user ? base[e] + user[e] : base[e];
+}
+
+// ---------------------------------------------------------------- K7 (PAPER.md:56 feedback)
+// x[r][:] = bf16( sum_i emb[i][tokens[r][i]][:] ), fp32 accumulation in stream order.  One CTA per
+// two-row slot; every thread owns 16-byte (8 x bf16) column chunks and keeps up to kFbUnroll
+// independent gathers in flight.  When both rows of the slot carry the same tokens (a CFG pair
+// after the token sync) the sum is formed once and stored twice.  HBM-bound:
+// 2 * S * d bytes gathered per distinct row + 2 * d bytes written per row.
+constexpr int kFbThreads = 256;
+constexpr int kFbUnroll = 8;
+
+__device__ __forceinline__ void fb_accumulate(float (&acc)[8], const uint4 v) {
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float2 f = __bfloat1622float2(h[q]);
+        acc[2 * q] += f.x;
+        acc[2 * q + 1] += f.y;
+    }
+}
+
+__global__ void __launch_bounds__(kFbThreads)
+cfgms_feedback_kernel(const int32_t* __restrict__ tokens, const __nv_bfloat16* __restrict__ emb,
+                      __nv_bfloat16* __restrict__ x, int R, int S, int V_e, int d) {
+    __shared__ int tok[2][64];
+    __shared__ int same_s;
+    const int r0 = 2 * blockIdx.x;
+    const int rows = min(2, R - r0);
+    if (threadIdx.x < 2 * S) {
+        const int rr = threadIdx.x / S, i = threadIdx.x - rr * S;
+        tok[rr][i] = rr < rows ? tokens[static_cast<size_t>(r0 + rr) * S + i] : -1;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int same = rows == 2;
+        for (int i = 0; i < S; ++i) same &= tok[0][i] == tok[1][i];
+        same_s = same;
+    }
+    __syncthreads();
+    const bool same = same_s != 0;
+    const int chunks = d >> 3;
+    for (int rr = 0; rr < (same ? 1 : rows); ++rr) {
+        for (int c = threadIdx.x; c < chunks; c += kFbThreads) {
+            float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            for (int i0 = 0; i0 < S; i0 += kFbUnroll) {
+                uint4 v[kFbUnroll];
+#pragma unroll
+                for (int u = 0; u < kFbUnroll; ++u) {
+                    const int i = i0 + u;
+                    const int t = i < S ? tok[rr][i] : -1;
+                    v[u] = (t >= 0 && t < V_e)
+                               ? __ldg(reinterpret_cast<const uint4*>(emb + (static_cast<size_t>(i) * V_e + t) * d) + c)
+                               : make_uint4(0u, 0u, 0u, 0u);      // bf16 +0: contributes nothing
+                }
+#pragma unroll
+                for (int u = 0; u < kFbUnroll; ++u) fb_accumulate(acc, v[u]);
+            }
+            uint4 o;
+            __nv_bfloat162* oh = reinterpret_cast<__nv_bfloat162*>(&o);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) oh[q] = __floats2bfloat162_rn(acc[2 * q], acc[2 * q + 1]);
+            reinterpret_cast<uint4*>(x + static_cast<size_t>(r0 + rr) * d)[c] = o;
+            if (same) reinterpret_cast<uint4*>(x + static_cast<size_t>(r0 + 1) * d)[c] = o;
+        }
+    }
+}
+
 }  // namespace cfgms

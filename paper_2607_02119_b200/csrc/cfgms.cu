@@ -31,6 +31,7 @@ struct HostStage {  // device staging for the *_host entry points
     int32_t *pair_map = nullptr, *top_k = nullptr, *step = nullptr, *n_frames = nullptr, *tokens = nullptr;
     float *w = nullptr, *temp = nullptr;
     uint32_t* req_id = nullptr;
+    int32_t *force_token = nullptr, *frame = nullptr, *frame_index = nullptr;
     int32_t* deint_in = nullptr;
     int32_t* deint_out = nullptr;
     size_t deint_in_bytes = 0, deint_out_bytes = 0;
@@ -44,7 +45,8 @@ struct cfgms_ctx {
     int max_rows = 0, pad_token = 0, row_tile_override = 0, max_stages = 0;
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     const __nv_bfloat16* heads = nullptr;
-    float* bias = nullptr;            // [NT]
+    float* bias = nullptr;            // [NT] what the epilogue adds: bias_base (+ the caller's logit bias)
+    float* bias_base = nullptr;       // [NT] W_i e_i, folded at create
     float* z = nullptr;               // [max_rows][NT]
     float* cand_val = nullptr;        // [max_rows][NT/32][4] top-4 per 32-token chunk (candidate path)
     uint32_t* cand_src = nullptr;     // [max_rows][NT/32]
@@ -124,6 +126,7 @@ int validate_step(const cfgms_ctx* c, const cfgms_step_args* a) {
     if (a->R < 1) return CFGMS_ERR_ARG;
     if (a->R > c->max_rows) return CFGMS_ERR_SHAPE;
     if (a->delayed && a->T_cap < 1) return CFGMS_ERR_ARG;
+    if ((a->frame_out || a->frame_index_out) && (!a->delayed || a->T_cap < c->S)) return CFGMS_ERR_ARG;
     return CFGMS_OK;
 }
 
@@ -194,6 +197,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
 
     int rc = CFGMS_OK;
     if ((rc = dev_alloc(&c->bias, static_cast<size_t>(c->NT))) != CFGMS_OK ||
+        (rc = dev_alloc(&c->bias_base, static_cast<size_t>(c->NT))) != CFGMS_OK ||
         (rc = dev_alloc(&c->z, static_cast<size_t>(c->max_rows) * c->NT)) != CFGMS_OK ||
         (rc = dev_alloc(&c->hidden_bf16, static_cast<size_t>(c->max_rows) * d)) != CFGMS_OK ||
         (rc = dev_alloc(&c->err, 2)) != CFGMS_OK ||
@@ -224,7 +228,8 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
         const int warps_per_block = 8;
         const int blocks = (c->NT + warps_per_block - 1) / warps_per_block;
         cfgms_bias_init_kernel<<<blocks, warps_per_block * 32>>>(c->heads, static_cast<const __nv_bfloat16*>(embeds),
-                                                                  c->bias, S, V, d);
+                                                                  c->bias_base, S, V, d);
+        cudaMemcpyAsync(c->bias, c->bias_base, static_cast<size_t>(c->NT) * sizeof(float), cudaMemcpyDeviceToDevice, 0);
         if (cudaDeviceSynchronize() != cudaSuccess) {
             cfgms_destroy(c);
             return CFGMS_ERR_CUDA;
@@ -269,6 +274,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
 void cfgms_destroy(cfgms_ctx* c) {
     if (!c) return;
     cudaFree(c->bias);
+    cudaFree(c->bias_base);
     cudaFree(c->z);
     cudaFree(c->cand_val);
     cudaFree(c->cand_src);
@@ -281,7 +287,8 @@ void cfgms_destroy(cfgms_ctx* c) {
     }
     HostStage& h = c->hs;
     cudaFree(h.hidden); cudaFree(h.pair_map); cudaFree(h.top_k); cudaFree(h.step); cudaFree(h.n_frames);
-    cudaFree(h.tokens); cudaFree(h.w); cudaFree(h.temp); cudaFree(h.req_id); cudaFree(h.deint_in); cudaFree(h.deint_out);
+    cudaFree(h.tokens); cudaFree(h.w); cudaFree(h.temp); cudaFree(h.req_id);
+    cudaFree(h.force_token); cudaFree(h.frame); cudaFree(h.frame_index); cudaFree(h.deint_in); cudaFree(h.deint_out);
     delete c;
 }
 
@@ -379,6 +386,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.pad_token = c->pad_token;
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
     fp.cand_val = c->cand_val; fp.cand_src = c->cand_src;
+    fp.force_token = a->force_token; fp.frame_out = a->frame_out; fp.frame_index_out = a->frame_index_out;
     fp.ready = gp.ready;
     fp.done = overlap ? c->ready + (c->ready_words - 33) : nullptr;
     fp.stats = overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 32)) : nullptr;
@@ -437,7 +445,8 @@ int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         const size_t R = static_cast<size_t>(c->max_rows);
         if (cudaMalloc(&h.hidden, R * c->d * 4) != cudaSuccess) return CFGMS_ERR_NOMEM;
         if (dev_alloc(&h.pair_map, R) || dev_alloc(&h.top_k, R) || dev_alloc(&h.step, R) || dev_alloc(&h.n_frames, R) ||
-            dev_alloc(&h.tokens, R * c->S) || dev_alloc(&h.w, R) || dev_alloc(&h.temp, R) || dev_alloc(&h.req_id, R))
+            dev_alloc(&h.tokens, R * c->S) || dev_alloc(&h.w, R) || dev_alloc(&h.temp, R) || dev_alloc(&h.req_id, R) ||
+            dev_alloc(&h.force_token, R * c->S) || dev_alloc(&h.frame, R * c->S) || dev_alloc(&h.frame_index, R))
             return CFGMS_ERR_NOMEM;
         c->hs_ready = true;
     }
@@ -452,19 +461,54 @@ int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
               up(h.temp, a->temp, R * 4) && up(h.top_k, a->top_k, R * 4) && up(h.step, a->step, R * 4);
     if (ok && a->req_id) ok = up(h.req_id, a->req_id, R * 4);
     if (ok && a->n_frames) ok = up(h.n_frames, a->n_frames, R * 4);
+    if (ok && a->force_token) ok = up(h.force_token, a->force_token, R * c->S * 4);
     if (!ok) return CFGMS_ERR_CUDA;
     cfgms_step_args d = *a;
     d.hidden = h.hidden; d.pair_map = h.pair_map; d.w = h.w; d.temp = h.temp; d.top_k = h.top_k; d.step = h.step;
     d.req_id = a->req_id ? h.req_id : nullptr;
     d.n_frames = a->n_frames ? h.n_frames : nullptr;
     d.tokens_out = h.tokens;
+    d.force_token = a->force_token ? h.force_token : nullptr;
+    d.frame_out = a->frame_out ? h.frame : nullptr;
+    d.frame_index_out = a->frame_index_out ? h.frame_index : nullptr;
     rc = cfgms_step(c, &d, cuda_stream);
     if (rc != CFGMS_OK) return rc;
     const size_t tok_bytes = R * c->S * 4;
     if (cudaMemcpyAsync(a->tokens_out, h.tokens, tok_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    int64_t d2h = static_cast<int64_t>(tok_bytes);
+    if (a->frame_out) {
+        if (cudaMemcpyAsync(a->frame_out, h.frame, tok_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+        d2h += static_cast<int64_t>(tok_bytes);
+    }
+    if (a->frame_index_out) {
+        if (cudaMemcpyAsync(a->frame_index_out, h.frame_index, R * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+        d2h += static_cast<int64_t>(R * 4);
+    }
     if (cudaStreamSynchronize(st) != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.h2d_bytes_last_step = h2d;
-    c->info.d2h_bytes_last_step = static_cast<int64_t>(tok_bytes);
+    c->info.d2h_bytes_last_step = d2h;
+    return CFGMS_OK;
+}
+
+int cfgms_set_logit_bias(cfgms_ctx* c, const float* bias, void* cuda_stream) {
+    if (!c) return CFGMS_ERR_ARG;
+    const int blocks = (c->NT + 255) / 256;
+    cfgms_bias_fold_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->bias_base, bias, c->bias, c->NT);
+    if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.launches_total += 1;
+    return CFGMS_OK;
+}
+
+int cfgms_feedback(cfgms_ctx* c, const int32_t* tokens, const void* emb, int32_t V_e, int32_t R, void* x_out,
+                   void* cuda_stream) {
+    if (!c || R < 0 || V_e < 1) return CFGMS_ERR_ARG;
+    if (R == 0) return CFGMS_OK;
+    if (!tokens || !emb || !x_out) return CFGMS_ERR_ARG;
+    if ((reinterpret_cast<uintptr_t>(emb) & 15u) != 0 || (reinterpret_cast<uintptr_t>(x_out) & 15u) != 0) return CFGMS_ERR_ARG;
+    cfgms_feedback_kernel<<<(R + 1) / 2, kFbThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        tokens, static_cast<const __nv_bfloat16*>(emb), static_cast<__nv_bfloat16*>(x_out), R, c->S, V_e, c->d);
+    if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.launches_total += 1;
     return CFGMS_OK;
 }
 

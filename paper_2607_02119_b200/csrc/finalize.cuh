@@ -42,6 +42,10 @@ struct FinalizeParams {
     const uint32_t* cand_src; // [R][NT/32]
     // Overlap with K1 (candidate path, V % 128 == 0): K1's epilogue warps count finished tiles per
     // (stream, row block) in ready[]; a cell is consumed once its group reached ready_target.
+    // widenings (all nullable): forced tokens, streaming frame emission (include/cfgms.h)
+    const int32_t* force_token;  // [R][S]
+    int32_t* frame_out;          // [R][S]
+    int32_t* frame_index_out;    // [R]
     int* ready;               // nullable [S][num_row_blocks]
     int* done;                // CTAs of this grid that finished; the last one clears ready[] for the next step
     unsigned long long* stats;// [16] cells that arrived before their group was complete (summed on the host)
@@ -94,6 +98,40 @@ __device__ __forceinline__ float key_float(uint32_t k) {
 __device__ __forceinline__ uint32_t float_key_fast(float f) {
     const uint32_t u = __float_as_uint(f);
     return u ^ (static_cast<uint32_t>(static_cast<int32_t>(u) >> 31) | 0x80000000u);
+}
+
+// Token of an ACTIVE cell given by the caller (phase machine hook), or -1.
+__device__ __forceinline__ int forced_token(const FinalizeParams& p, int r, int i) {
+    return p.force_token ? p.force_token[static_cast<size_t>(r) * p.S + i] : -1;
+}
+
+// Rows a4 of the hot path, by ONE thread per cell: token to the row and its companion
+// (PAPER.md:93), delayed-layout cell.  The thread of the LAST stream also emits
+// the frame that completes at this step: f = tau - S + 1, frame[i] = ring[(f + i) mod
+// T_cap][i]; streams i < S - 1 were written by earlier steps' launches, stream S - 1 is `token`.
+__device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i, int pm, int tau, int token) {
+    p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
+    if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
+    if (p.delayed) {
+        const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
+        p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
+    }
+    if (i == p.S - 1 && (p.frame_out || p.frame_index_out)) {
+        const int f = tau - p.S + 1;
+        const bool done = f >= 0 && (p.n_frames == nullptr || f < p.n_frames[r]) && p.delayed && p.T_cap >= p.S;
+        if (p.frame_index_out) {
+            p.frame_index_out[r] = done ? f : -1;
+            if (pm >= 0) p.frame_index_out[pm] = -1;
+        }
+        if (p.frame_out) {
+            int32_t* fr = p.frame_out + static_cast<size_t>(r) * p.S;
+            const int32_t* ring = p.delayed + static_cast<size_t>(r) * p.T_cap * p.S;
+            for (int j = 0; j < p.S; ++j)
+                fr[j] = !done ? p.pad_token : j == p.S - 1 ? token : ring[static_cast<size_t>((f + j) % p.T_cap) * p.S + j];
+            if (pm >= 0)
+                for (int j = 0; j < p.S; ++j) p.frame_out[static_cast<size_t>(pm) * p.S + j] = p.pad_token;
+        }
+    }
 }
 
 struct BestSV {
@@ -192,8 +230,12 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
     if (pm >= 0 && (r & 1)) return;  // companion row: its cond row writes both
 
     const int tau = p.step[r];
-    const bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
     int token = p.pad_token;
+    if (active) {
+        const int ft = forced_token(p, r, i);
+        if (ft >= 0) { token = ft; active = false; }
+    }
 
     if (active) {
         const int V = p.V;
@@ -283,14 +325,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
         best = block_argmax(best, red_s, red_v);
         token = best.v;
     }
-    if (tid == 0) {
-        p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
-        if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
-        if (p.delayed) {
-            const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
-            p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
-        }
-    }
+    if (tid == 0) write_cell(p, r, i, pm, tau, token);
 }
 
 // Fallback for V > 256 * 32: keys in shared memory, radix select over all of them.
@@ -305,8 +340,12 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
     const int pm = p.pair_map[r];
     if (pm >= 0 && (r & 1)) return;
     const int tau = p.step[r];
-    const bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
     int token = p.pad_token;
+    if (active) {
+        const int ft = forced_token(p, r, i);
+        if (ft >= 0) { token = ft; active = false; }
+    }
     if (active) {
         const int V = p.V;
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
@@ -337,14 +376,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
         best = block_argmax(best, red_s, red_v);
         token = best.v;
     }
-    if (tid == 0) {
-        p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
-        if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
-        if (p.delayed) {
-            const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
-            p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
-        }
-    }
+    if (tid == 0) write_cell(p, r, i, pm, tau, token);
 }
 
 
@@ -407,8 +439,12 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     int* list_v = reinterpret_cast<int*>(list_key + cap);
 
     const int tau = p.step[r];
-    const bool active = valid && (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    bool active = valid && (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
     int token = p.pad_token;
+    if (active) {
+        const int ft = forced_token(p, r, i);
+        if (ft >= 0) { token = ft; active = false; }
+    }
     if (active) {
         if (p.ready) {
             // wait until K1 has written every tile of this (stream, row block): acquire pairs with
@@ -636,14 +672,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         best = warp_argmax(best);
         token = best.v;
     }
-    if (valid && lane == 0) {
-        p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
-        if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
-        if (p.delayed) {
-            const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
-            p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
-        }
-    }
+    if (valid && lane == 0) write_cell(p, r, i, pm, tau, token);
     if (p.ready) {
         // the last CTA to finish re-arms the counters for the next step's K1 (which starts after this grid)
         __syncthreads();

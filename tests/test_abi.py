@@ -35,13 +35,28 @@ def test_version_and_strerror_strings():
     assert b"fallback" in lib.cfgms_strerror(5)
 
 
-def test_struct_layouts_match_header():
-    # sizes the C compiler gives the ABI structs (LP64): guards the ctypes mirrors
+def test_struct_layouts_match_header(tmp_path):
+    # the C compiler's view of include/cfgms.h (LP64) against the ctypes mirrors, field by field
+    import os
+    import subprocess
     from paper_2607_02119_b200 import binding as b
-    assert C.sizeof(b.cfgms_config) == 32
-    assert C.sizeof(b.cfgms_step_args) == 112
-    assert b.cfgms_step_args.seed.offset == 48 and b.cfgms_step_args.T_cap.offset == 96
-    assert C.sizeof(b.cfgms_info) == 80
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    structs = {"cfgms_config": b.cfgms_config, "cfgms_step_args": b.cfgms_step_args, "cfgms_info": b.cfgms_info}
+    lines = []
+    for name, cls in structs.items():
+        lines.append(f'printf("{name} %zu\\n", sizeof({name}));')
+        for field, _ in cls._fields_:
+            lines.append(f'printf("{name}.{field} %zu\\n", offsetof({name}, {field}));')
+    src = tmp_path / "layout.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "cfgms.h"\nint main(void) {\n' + "\n".join(lines) + "\nreturn 0; }\n")
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-std=c99", "-I", os.path.join(root, "include"), "-o", str(exe), str(src)], check=True)
+    out = dict(l.split() for l in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
+    for name, cls in structs.items():
+        assert int(out[name]) == C.sizeof(cls), name
+        for field, _ in cls._fields_:
+            assert int(out[f"{name}.{field}"]) == getattr(cls, field).offset, f"{name}.{field}"
+    assert C.sizeof(b.cfgms_step_args) == 136 and b.cfgms_step_args.seed.offset == 48
 
 
 def test_create_without_gpu_fails_loudly():

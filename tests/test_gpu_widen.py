@@ -1,0 +1,195 @@
+"""GPU parity of the widenings against the oracle, through the C ABI:
+W1 streaming frame emission (bit-exact), W2 static logit bias + forced tokens (same tolerance
+rules as the main path), W3 feedback aggregation (correctly rounded bf16 of the exact sum)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads
+from parity_util import LOGIT_TOL, DeviceWorkload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dev():
+    return torch.device("cuda:0")
+
+
+def _custom(pairs, singles, d, S, V, T=16, mixed=False, **kw):
+    ov = dict(pairs=pairs, singles=singles, d=d, S=S, V=V, T=T, mixed=mixed, hidden_f32=False, heavy_tail=False)
+    ov.update(kw)
+    return workloads.make_config(2 if not mixed else 4, overrides=ov)
+
+
+# ------------------------------------------------------------------ W1
+@pytest.mark.parametrize("case", [
+    dict(wl=("config", 1), T_cap=None, no_candidates=False),          # full delayed matrix
+    dict(wl=("config", 1), T_cap=4, no_candidates=False),             # ring of depth exactly S
+    dict(wl=("config", 1), T_cap=7, no_candidates=True),              # full-scan sampler kernel
+    dict(wl=("custom", dict(pairs=3, singles=4, d=128, S=9, V=160, T=30)), T_cap=9, no_candidates=False),
+    dict(wl=("custom", dict(pairs=1, singles=2, d=64, S=1, V=64, T=6)), T_cap=1, no_candidates=False),
+])
+def test_streaming_frames_equal_the_deinterleaved_grid(dev, case):
+    kind, arg = case["wl"]
+    wl = workloads.make_config(arg) if kind == "config" else _custom(**arg)
+    dw = DeviceWorkload(wl, dev, T_cap=case["T_cap"], no_candidates=case["no_candidates"])
+    full = DeviceWorkload(wl, dev)                  # keeps the whole delayed matrix for the bulk de-interleave
+    R, S, pad = wl.R, wl.S, wl.pad_token
+    nf = wl.n_frames.numpy() if wl.n_frames is not None else None
+    heads = wl.head_rows()
+    pm = wl.pair_map.numpy()
+    frames = {int(c): {} for c in heads}
+    for t in range(wl.T):
+        frame = torch.full((R, S), -9, dtype=torch.int32, device=dev)
+        fidx = torch.full((R,), -9, dtype=torch.int32, device=dev)
+        st = wl.step(t).to(dev)
+        dw.ctx.step(dw.hidden(t), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, st, dw.tokens, req_id=dw.req_id,
+                    n_frames=dw.n_frames, delayed=dw.delayed, frame_out=frame, frame_index_out=fidx)
+        full.step(t)
+        dw.check_no_device_error()
+        fr, fi, ring = frame.cpu().numpy(), fidx.cpu().numpy(), dw.delayed.cpu().numpy()
+        tau = wl.step(t).numpy()
+        for c in heads:
+            # the oracle's emission rule applied to the GPU's own ring (integer work: bit-exact)
+            want_f, want_fr = oracle.emit_frame(ring[c], int(tau[c]), int(nf[c]) if nf is not None else -1, pad)
+            assert fi[c] == want_f and np.array_equal(fr[c], want_fr), (t, c)
+            if want_f >= 0:
+                frames[int(c)][want_f] = fr[c].copy()
+            if pm[c] >= 0:      # companion outputs stay hidden
+                assert fi[pm[c]] == -1 and np.all(fr[pm[c]] == pad)
+    # all frames of a request, in order, are exactly the bulk de-interleave of its delayed matrix
+    grid = oracle.deinterleave(full.delayed.cpu().numpy()[heads])
+    for q, c in enumerate(heads):
+        F = grid.shape[1] if nf is None else min(int(nf[c]), grid.shape[1])
+        got = frames[int(c)]
+        tau0 = int(wl.step(0).numpy()[c])
+        want_ids = [f for f in range(F) if tau0 <= f + S - 1 < tau0 + wl.T]      # frames completing inside the window
+        assert sorted(got) == want_ids
+        if tau0 == 0:
+            for f in want_ids:
+                assert np.array_equal(got[f], grid[q, f]), (c, f)
+
+
+def test_frame_emission_needs_a_ring_of_depth_S(dev):
+    import paper_2607_02119_b200 as pkg
+    wl = workloads.make_config(1)
+    dw = DeviceWorkload(wl, dev, T_cap=2)
+    frame = torch.zeros((wl.R, wl.S), dtype=torch.int32, device=dev)
+    with pytest.raises(pkg.CfgmsError) as e:
+        dw.ctx.step(dw.hidden(0), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, wl.step(0).to(dev), dw.tokens,
+                    delayed=dw.delayed, frame_out=frame)
+    assert e.value.status == 1      # CFGMS_ERR_ARG
+
+
+# ------------------------------------------------------------------ W2
+def _compare_ext(dw, t, logit_bias=None, force_token=None):
+    """One GPU step with the widening inputs against oracle.step(...) with the same inputs."""
+    wl, dev = dw.wl, dw.dev
+    logits = torch.zeros((wl.R, wl.S, wl.V), dtype=torch.float32, device=dev)
+    dw.tokens.fill_(-1)
+    ft_dev = None if force_token is None else torch.from_numpy(force_token).to(dev)
+    dw.ctx.step(dw.hidden(t), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, wl.step(t).to(dev), dw.tokens,
+                req_id=dw.req_id, n_frames=dw.n_frames, delayed=dw.delayed, logits_out=logits, force_token=ft_dev)
+    dw.check_no_device_error()
+    ref = oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, wl.step(t),
+                      wl.req_id, wl.n_frames, wl.pad_token, want_merged=True, hidden_is_f32=wl.hidden_f32,
+                      logit_bias=logit_bias, force_token=force_token)
+    got, gl = dw.tokens.cpu().numpy(), logits.cpu().numpy().astype(np.float64)
+    pm = wl.pair_map.numpy()
+    n_close = n_forced = 0
+    for j, (c, i) in enumerate(ref.cells):
+        fl = int(ref.flags[j])
+        if pm[c] >= 0:
+            assert got[pm[c], i] == got[c, i]
+        if fl & oracle.FLAG_INACTIVE:
+            assert got[c, i] == wl.pad_token
+        elif fl & oracle.FLAG_FORCED:
+            n_forced += 1
+            assert got[c, i] == force_token[c, i]
+        else:
+            m = ref.merged[j]
+            fin = np.isfinite(m)
+            assert np.array_equal(np.isneginf(gl[c, i]), np.isneginf(m))          # masked tokens are -inf on both sides
+            assert np.max(np.abs(gl[c, i][fin] - m[fin])) <= LOGIT_TOL
+            if fl & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
+                n_close += 1
+            else:
+                assert got[c, i] == ref.tok[j], (t, c, i, got[c, i], ref.tok[j], ref.margin[j])
+            assert np.isfinite(m[got[c, i]])                                        # never a masked token
+    return n_close, n_forced
+
+
+@pytest.mark.parametrize("no_candidates", [False, True])
+def test_logit_bias_masks_and_forced_tokens(dev, no_candidates):
+    wl = _custom(pairs=6, singles=4, d=256, S=4, V=512, T=16, mixed=True, top_k=20)
+    dw = DeviceWorkload(wl, dev, no_candidates=no_candidates)
+    rng = np.random.default_rng(12)
+    bias = rng.normal(scale=0.5, size=(wl.S, wl.V))
+    bias[0, 100:] = -np.inf                     # stream 0 may only use its first 100 tokens (< top_k survivors stay finite)
+    bias[1, rng.random(wl.V) < 0.5] = -np.inf   # scattered mask
+    bias[2, 7:] = -np.inf                       # 7 tokens left: fewer than top_k
+    bias[3, :] = 0.0
+    ft = np.full((wl.R, wl.S), -1, dtype=np.int32)
+    for c in wl.head_rows()[::3]:
+        ft[c, 1] = 300 + int(c)                 # bridging token on stream 1
+        ft[c, 3] = wl.pad_token                 # text-phase padding on stream 3
+    dw.ctx.set_logit_bias(torch.from_numpy(bias.astype(np.float32)).to(dev))
+    bias32 = bias.astype(np.float32).astype(np.float64)      # the oracle sees the same fp32 values
+    n_forced = 0
+    for t in (0, 2, 5, 9):
+        _, nf = _compare_ext(dw, t, logit_bias=bias32, force_token=ft)
+        n_forced += nf
+    assert n_forced > 0
+    # clearing the bias restores the plain path
+    dw.ctx.set_logit_bias(None)
+    _compare_ext(dw, 5)
+
+
+def test_logit_bias_on_config2_shape_in_the_bench_launch_configuration(dev):
+    wl = workloads.make_config(2)
+    dw = DeviceWorkload(wl, dev)
+    rng = np.random.default_rng(3)
+    bias = np.where(rng.random((wl.S, wl.V)) < 0.3, -np.inf, 0.0) + rng.normal(scale=0.2, size=(wl.S, wl.V))
+    dw.ctx.set_logit_bias(torch.from_numpy(bias.astype(np.float32)).to(dev))
+    n_close, _ = _compare_ext(dw, 40, logit_bias=bias.astype(np.float32).astype(np.float64))
+    assert n_close < 0.08 * wl.n_req * wl.S
+
+
+# ------------------------------------------------------------------ W3
+def _bf16_ulp(x):
+    """Spacing of bf16 (8 significand bits) at |x| (float64 array)."""
+    ax = np.maximum(np.abs(x), 2.0 ** -126)
+    return 2.0 ** (np.floor(np.log2(ax)) - 7)
+
+
+@pytest.mark.parametrize("shape", [
+    dict(R=7, S=3, V_e=50, d=64),            # odd row count, one 16-byte chunk per 8 columns
+    dict(R=64, S=9, V_e=257, d=2048),        # OpusLM-like 9 streams
+    dict(R=256, S=16, V_e=2049, d=4096),     # config-5 head shape (V + 1 rows: PAD has an embedding)
+])
+def test_feedback_is_the_correctly_rounded_sum(dev, shape):
+    R, S, V_e, d = shape["R"], shape["S"], shape["V_e"], shape["d"]
+    g = torch.Generator().manual_seed(R + S)
+    emb = (torch.randn(S, V_e, d, generator=g) * 0.5).to(torch.bfloat16)
+    tok = torch.randint(0, V_e, (R, S), generator=g, dtype=torch.int32)
+    tok[1::2] = tok[0::2][: tok[1::2].shape[0]]          # companion rows carry their cond row's tokens
+    if R > 4:
+        tok[4, 0] = -1                                    # ids outside [0, V_e) contribute nothing
+        tok[4, S - 1] = V_e
+        tok[3, 1] = (tok[3, 1] + 1) % V_e                 # a slot whose two rows differ
+    heads = torch.zeros(S, 128, d, dtype=torch.bfloat16, device=dev)
+    import paper_2607_02119_b200 as pkg
+    ctx = pkg.Context(heads, torch.zeros(S, d, dtype=torch.bfloat16, device=dev), max_rows=8)
+    x = ctx.feedback(tok.to(dev), emb.to(dev))
+    torch.cuda.synchronize()
+    got = x.float().cpu().numpy().astype(np.float64)
+    want = oracle.feedback(tok.numpy(), emb)
+    # fp32 accumulation of S bf16 terms then one RNE to bf16: within half a bf16 ulp of the exact sum,
+    # plus the fp32 accumulation error (S * 2^-24 * sum of |terms| <= S * 2^-24 * S * max|term|)
+    terms_max = float(emb.float().abs().max())
+    tol = 0.5 * _bf16_ulp(want) * (1 + 1e-6) + S * S * 2.0 ** -24 * terms_max
+    assert np.all(np.abs(got - want) <= tol), float(np.max(np.abs(got - want) / _bf16_ulp(want)))
+    assert np.array_equal(got[1][: d], got[0][: d]) if R >= 2 else True
+    ctx.close()
