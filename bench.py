@@ -207,6 +207,49 @@ class Runner:
         times.sort()
         return times[len(times) // 2]
 
+    def time_widenings(self, K: int):
+        """Widening kernels at this config: feedback gather-sum alone (CUDA
+        events, tables larger than L2), and the step with streaming frame emission switched on."""
+        torch = self.torch
+        wl = self.wl
+        g = torch.Generator().manual_seed(7)
+        emb = (torch.randn(wl.S, wl.V + 1, wl.d, generator=g, dtype=torch.float32) * 0.05).to(torch.bfloat16).to(self.dev)
+        x = torch.empty((wl.R, wl.d), dtype=torch.bfloat16, device=self.dev)
+        self.step(wl.S)
+        for _ in range(3):
+            self.ctx.feedback(self.tokens, emb, x)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for j in range(K):
+            self.step(wl.S + j)          # fresh tokens every iteration: different rows gathered
+            self.ctx.feedback(self.tokens, emb, x)
+        e1.record()
+        torch.cuda.synchronize()
+        both = e0.elapsed_time(e1) * 1e3 / K
+        e0.record()
+        for j in range(K):
+            self.step(wl.S + j)
+        e1.record()
+        torch.cuda.synchronize()
+        alone = e0.elapsed_time(e1) * 1e3 / K
+        fb_us = max(both - alone, 1e-3)
+        # distinct rows gathered once (a companion row repeats its cond row's tokens) + x written for every row
+        fb_bytes = 2.0 * wl.n_req * wl.S * wl.d + 2.0 * wl.R * wl.d
+        frame = torch.empty((wl.R, wl.S), dtype=torch.int32, device=self.dev)
+        fidx = torch.empty((wl.R,), dtype=torch.int32, device=self.dev)
+        e0.record()
+        for j in range(K):
+            t = wl.S + j
+            self.ctx.step(self.pool[t % self.pool.shape[0]], self.pair_map, self.w, self.temp, self.top_k, wl.seed,
+                          self.steps_dev[t % wl.T], self.tokens, req_id=self.req_id, n_frames=self.n_frames,
+                          delayed=self.delayed, frame_out=frame, frame_index_out=fidx)
+        e1.record()
+        torch.cuda.synchronize()
+        with_frames = e0.elapsed_time(e1) * 1e3 / K
+        del emb
+        return {"feedback_us": fb_us, "feedback_algorithmic_bytes": fb_bytes, "feedback_gbs": fb_bytes / fb_us / 1e3,
+                "step_us_eager": alone, "step_with_frame_emission_us_eager": with_frames}
+
     def time_e2e(self, K: int, warmup: int):
         """Same step through cfgms_step_host: pinned host inputs in, host tokens out, every step."""
         torch = self.torch
@@ -386,6 +429,9 @@ def main():
         cb, _, _ = oracle_sample(wl)
         line["cpu_baseline"] = cb
         if not args.no_extras:
+            wd = main_r.time_widenings(50)
+            wd["feedback_frac_of_hbm_peak"] = wd["feedback_gbs"] / peaks["hbm_gbs"]
+            line["widenings"] = wd
             del main_r
             torch.cuda.empty_cache()
             flush = torch.zeros(256 * 2 ** 20 // 4, dtype=torch.int32, device=dev)

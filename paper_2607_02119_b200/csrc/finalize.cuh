@@ -445,25 +445,27 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         const int ft = forced_token(p, r, i);
         if (ft >= 0) { token = ft; active = false; }
     }
-    if (active) {
-        if (p.ready) {
-            // wait until K1 has written every tile of this (stream, row block): acquire pairs with
-            // the epilogue warps' red.release; bounded so a pipeline bug fails loudly
-            const int* flag = p.ready + i * p.num_row_blocks + r / p.BN;
-            if (lane == 0 && ld_acquire_gpu(flag) < p.ready_target) {
-                atomicAdd(p.stats + (blockIdx.x & 15), 1ull);   // evidence counter, spread over 16 words
-                const uint64_t t0 = global_timer_ns();
-                while (ld_acquire_gpu(flag) < p.ready_target) {
-                    __nanosleep(200);
-                    if (global_timer_ns() - t0 > 2000000000ull) {
-                        atomicCAS(p.err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (9 << 8));
-                        __threadfence_system();
-                        __trap();
-                    }
+    if (valid && p.ready) {
+        // Wait until K1 has written every tile of this (stream, row block): the acquire pairs with the
+        // epilogue warps' red.release.  EVERY request-owning cell waits, also a PAD or forced one that
+        // reads nothing: the last CTA of this grid re-arms the counters, which is only safe once
+        // every group is complete, i.e. once K1 will not signal again.  Bounded: a pipeline bug fails loudly.
+        const int* flag = p.ready + i * p.num_row_blocks + r / p.BN;
+        if (lane == 0 && ld_acquire_gpu(flag) < p.ready_target) {
+            atomicAdd(p.stats + (blockIdx.x & 15), 1ull);   // evidence counter, spread over 16 words
+            const uint64_t t0 = global_timer_ns();
+            while (ld_acquire_gpu(flag) < p.ready_target) {
+                __nanosleep(200);
+                if (global_timer_ns() - t0 > 2000000000ull) {
+                    atomicCAS(p.err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (9 << 8));
+                    __threadfence_system();
+                    __trap();
                 }
             }
-            __syncwarp();
         }
+        __syncwarp();
+    }
+    if (active) {
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
         const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
         const float temp = p.temp[r];

@@ -355,20 +355,30 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 float* zp = p.z + static_cast<size_t>(row_base) * NT + n;
                 float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
                 int any_odd = 0;
-                // ---- pass A: the request at the even row of every slot
+                // ---- pass A: the request at the even row of every slot.  Row pointers advance by a
+                // fixed stride so that the stores stay predicated (no per-row address rebuild, no branch).
+                const int own_even = n_ok ? 1 : 0, own_odd = n_ok ? 2 : 0;   // kind bits this thread may act on
+                const size_t row_stride = 2 * NT * sizeof(float);      // bytes between the even rows of two slots
+                {
+                    char* zq = reinterpret_cast<char*>(zp);
+                    char* tq = reinterpret_cast<char*>(tp);
+                    asm volatile("" : "+l"(zq));      // one running per-thread pointer, not base + offset pairs
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const SlotCoefA c = ca[j];
-                    const float a0 = __uint_as_float(v[2 * j]);
-                    const float a1 = __uint_as_float(v[2 * j + 1]);
-                    const float z0 = fmaf(c.c00, a0, fmaf(c.c01, a1, bias * c.d0));
-                    const bool own = n_ok && (c.kind & 1);
-                    any_odd |= c.kind;
-                    if (own) {
-                        zp[static_cast<size_t>(2 * j) * NT] = z0;
-                        if (kTap) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
+                    for (int j = 0; j < 32; ++j) {
+                        const SlotCoefA c = ca[j];
+                        const float a0 = __uint_as_float(v[2 * j]);
+                        const float a1 = __uint_as_float(v[2 * j + 1]);
+                        const float z0 = fmaf(c.c00, a0, fmaf(c.c01, a1, bias * c.d0));
+                        const bool own = (c.kind & own_even) != 0;
+                        any_odd |= c.kind;
+                        if (own) st_global_f32(zq, z0);
+                        if (kTap) {
+                            if (own) { const SlotCoefB t = cb[j]; *reinterpret_cast<float*>(tq) = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
+                            tq += row_stride;
+                        }
+                        zq += row_stride;
+                        if (kCand) stg[j * kStgPitch + lane] = own ? z0 + 0.0f : -INFINITY;
                     }
-                    if (kCand) stg[j * kStgPitch + lane] = own ? z0 + 0.0f : -INFINITY;
                 }
                 if (kCand) {
                     __syncwarp();
@@ -383,17 +393,22 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 }
                 // ---- pass B: slots that hold two unpaired rows — the request at the odd row
                 if (any_odd & 2) {
+                    char* zq = reinterpret_cast<char*>(zp + NT);
+                    char* tq = kTap ? reinterpret_cast<char*>(tp + NT) : nullptr;
+                    asm volatile("" : "+l"(zq));
 #pragma unroll
                     for (int j = 0; j < 32; ++j) {
                         const int kind = ca[j].kind;
                         const SlotCoefB c = cb[j];
                         const float a1 = __uint_as_float(v[2 * j + 1]);
                         const float z1 = fmaf(c.c11, a1, bias * c.d1);
-                        const bool own = n_ok && (kind & 2);
-                        if (own) {
-                            zp[static_cast<size_t>(2 * j + 1) * NT] = z1;
-                            if (kTap) tp[static_cast<size_t>(2 * j + 1) * NT] = a1 + bias;
+                        const bool own = (kind & own_odd) != 0;
+                        if (own) st_global_f32(zq, z1);
+                        if (kTap) {
+                            if (own) *reinterpret_cast<float*>(tq) = a1 + bias;
+                            tq += row_stride;
                         }
+                        zq += row_stride;
                         if (kCand) stg[j * kStgPitch + lane] = own ? z1 + 0.0f : -INFINITY;
                     }
                     if (kCand) {

@@ -342,3 +342,21 @@ def test_overlapped_finalize_equals_serial_finalize(dev):
         torch.cuda.synchronize()
         assert torch.equal(ov.tokens, ser.tokens)
     ov.check_no_device_error()
+
+
+def test_overlap_counters_survive_steps_whose_cells_are_mostly_pad(dev):
+    """Regression: at tau = 0 only stream 0 samples; if PAD cells did not wait for their group the
+    finalize grid could finish (and re-arm the ready counters) while the GEMM was still signalling,
+    and the NEXT step would read unfinished tiles.  Multi-wave overlapped GEMM (8 row blocks x 64
+    vocabulary tiles), PAD-heavy and full steps alternating, against the strictly serial launch."""
+    wl = _custom(pairs=256, singles=0, d=512, S=8, V=1024, T=64)
+    ov = DeviceWorkload(wl, dev, row_tile=64, force_overlap=True)
+    ser = DeviceWorkload(wl, dev, no_overlap=True)
+    for rep in range(12):
+        for t in (0, 9, 1, 30, wl.T - 1, 12):
+            ov.step(t)
+            ser.step(t)
+            torch.cuda.synchronize()
+            assert torch.equal(ov.tokens, ser.tokens), (rep, t)
+    assert ov.ctx.info()["overlap"] == 1
+    ov.check_no_device_error()
