@@ -58,6 +58,8 @@ def lib():
         L.oracle_emit_frame.argtypes = [C.c_void_p] + [C.c_int32] * 5 + [C.c_void_p]
         L.oracle_feedback.restype = None
         L.oracle_feedback.argtypes = [C.c_void_p, C.c_void_p] + [C.c_int32] * 4 + [C.c_void_p]
+        L.oracle_advance_state.restype = C.c_int32
+        L.oracle_advance_state.argtypes = [C.c_int32] * 6 + [C.c_void_p, C.c_void_p]
         L.oracle_logits_row.restype = None
         L.oracle_logits_row.argtypes = [C.c_void_p] * 3 + [C.c_int32] * 5 + [C.c_void_p]
         L.oracle_cfg_merge.restype = None
@@ -276,3 +278,13 @@ def feedback(tokens, emb) -> np.ndarray:
     x = np.empty((R, d), dtype=np.float64)
     lib().oracle_feedback(_p(tk), _p(eb), R, S, V_e, d, _p(x))
     return x
+
+
+F_UNSET = 2 ** 31 - 1   # "no frame count yet": every stream i <= tau stays active
+
+
+def advance_state(tau: int, F: int, tok0: int, eos: int, S: int):
+    """Widening W4 -> (tau_next, F_next, drained)."""
+    tn, fn = C.c_int32(), C.c_int32()
+    done = lib().oracle_advance_state(int(tau), int(F), int(tok0), int(eos), int(S), F_UNSET, C.byref(tn), C.byref(fn))
+    return int(tn.value), int(fn.value), bool(done)

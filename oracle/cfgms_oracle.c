@@ -39,6 +39,9 @@
  *      reduced vocabulary (chi-square vs softmax over the unmasked tokens); forced cells verbatim
  *   W3 oracle_feedback     sum of the sampled tokens' stream embeddings
  *      pin: torch fp64 gather-sum; one stream == row copy; out-of-range ids contribute zero
+ *   W4 oracle_advance_state  step counter, frame count set by end-of-audio, drained flag
+ *      pin: a request driven by it to completion produces exactly interleave(grid of F frames):
+ *      S(S-1)/2 PAD cells at each end, F + S - 1 steps, S - 1 PADs on the primary stream in the drain
  */
 #include <math.h>
 #include <stdint.h>
@@ -396,6 +399,24 @@ void oracle_feedback(const int32_t* tokens, const uint16_t* emb, int32_t R, int3
             }
             x[(size_t)r * d + k] = acc;
         }
+}
+
+/* Widening W4 — device-resident request state with automatic drain ("terminating the
+ * audio phase initiates a drain sub-phase that emits S-1 padding tokens to flush the delay buffer,
+ * guaranteeing a complete S x T codebook matrix"; reading C27: the audio phase of a request ends
+ * when its PRIMARY stream (stream 0) emits the end-of-audio token at step tau; the frames completed
+ * so far, F = tau, become the request's frame count, stream 0 pads from then on and stream i keeps
+ * sampling its delayed tokens for i more steps).  `unset` marks "no frame count yet".
+ *   in : tau, F (or unset), tok0 = the token stream 0 emitted at this step, eos (< 0: none)
+ *   out: *tau_next = tau + 1;  *F_next = F, or tau if F was unset and tok0 == eos;
+ *        returns 1 iff the request is fully drained after this step: tau + 1 >= F_next + S - 1. */
+int32_t oracle_advance_state(int32_t tau, int32_t F, int32_t tok0, int32_t eos, int32_t S, int32_t unset,
+                             int32_t* tau_next, int32_t* F_next) {
+    int32_t Fn = F;
+    if (F == unset && eos >= 0 && tok0 == eos) Fn = tau;
+    *tau_next = tau + 1;
+    *F_next = Fn;
+    return (Fn != unset && tau + 1 >= Fn + S - 1) ? 1 : 0;
 }
 
 /* ---- test helper: empirical token frequencies of O6-O8 on fixed merged logits ------------- */

@@ -175,3 +175,53 @@ def test_forced_tokens_are_emitted_verbatim_and_only_in_active_cells():
         else:
             assert ext.tok[j] == base.tok[j] and ext.flags[j] == base.flags[j]
     assert tokens[0, 1] == 200 and tokens[1, 1] == 200      # synchronised to the companion
+
+
+# ------------------------------------------------------------------ W4: device-resident state, automatic drain
+def test_state_machine_drives_a_request_to_a_complete_codebook_matrix():
+    """ending the audio phase starts a drain that emits S-1 paddings on the primary stream and
+    guarantees a complete matrix.  Drive one request with oracle.advance_state only (tokens are arbitrary
+    symbols here; the end-of-audio symbol appears on stream 0 at a chosen step) and check the result
+    against the interleave rule written out independently: F frames, F + S - 1 steps, PAD exactly
+    where t - i is outside [0, F)."""
+    EOS, PAD = 777, 1000
+    for S in (1, 2, 4, 9):
+        for F_true in (0, 1, 3, 11):
+            tau, F, rows, done, steps = 0, oracle.F_UNSET, [], False, 0
+            while not done:
+                row = []
+                for i in range(S):
+                    active = i <= tau and (tau - i < F)          # activity rule O5 with the CURRENT frame count
+                    tok = PAD if not active else (EOS if (i == 0 and tau == F_true) else 10 * tau + i)
+                    row.append(tok)
+                rows.append(row)
+                tau, F, done = oracle.advance_state(tau, F, row[0], EOS, S)
+                steps += 1
+                assert steps < 200
+            assert F == F_true
+            # the end-of-audio step itself plus S - 2 further drain steps (none to flush when S <= 2)
+            assert steps == max(F_true + 1, F_true + S - 1)
+            D = np.array(rows, dtype=np.int64)
+            for t in range(D.shape[0]):
+                for i in range(S):
+                    f = t - i
+                    if 0 <= f < F_true:
+                        assert D[t, i] == 10 * t + i
+                    elif i == 0 and t == F_true:
+                        assert D[t, i] == EOS            # the end-of-audio symbol itself, never part of a frame
+                    else:
+                        assert D[t, i] == PAD
+            if S > 1 and F_true > 0:
+                # S - 1 paddings on the primary stream during the drain (the EOS step aside)
+                assert (D[F_true + 1:, 0] == PAD).sum() == S - 2 and D.shape[0] == F_true + S - 1
+                # and the de-interleaved matrix is complete: no PAD, no EOS inside the F frames
+                dl = np.full((1, F_true + S - 1, S), PAD, dtype=np.int32)
+                dl[0, :D.shape[0]] = D
+                grid = oracle.deinterleave(dl)[0]
+                assert grid.shape == (F_true, S) and (grid != PAD).all() and (grid != EOS).all()
+
+
+def test_state_machine_ignores_eos_without_an_eos_id_and_after_the_frame_count_is_set():
+    assert oracle.advance_state(3, oracle.F_UNSET, 5, -1, 4) == (4, oracle.F_UNSET, False)
+    assert oracle.advance_state(6, 2, 5, 5, 4) == (7, 2, True)         # F stays 2 although stream 0 shows the id again
+    assert oracle.advance_state(0, oracle.F_UNSET, 5, 5, 4) == (1, 0, False)   # end of audio before any frame
