@@ -129,7 +129,21 @@ typedef struct {
                                  with T_cap >= S (else CFGMS_ERR_ARG).  Companion rows: pad      */
     int32_t* frame_index_out; /* [R] the frame index f emitted for the row, or -1 (also -1 at
                                  companion rows, whose outputs stay hidden)         */
+    /* device-resident request state with automatic drain.  With these three the
+       decode loop needs no host bookkeeping: feed step_next_out / n_frames_next_out of one step
+       as step / n_frames of the next (two buffers, alternating).  Written at cond / unpaired rows. */
+    int32_t eos_token;        /* end-of-audio id on the PRIMARY stream (stream 0); < 0 = none.  When
+                                 stream 0 emits it at step tau while the request's frame count is
+                                 still CFGMS_FRAMES_UNSET, the frame count becomes tau: stream 0
+                                 pads from the next step on, stream i keeps sampling i more steps  */
+    int32_t* step_next_out;   /* [R] tau + 1                                                       */
+    int32_t* n_frames_next_out; /* [R] the frame count after this step (CFGMS_FRAMES_UNSET until the
+                                 end-of-audio token appears; n_frames == NULL reads as UNSET)       */
+    int32_t* done_out;        /* [R] 1 when the request is fully drained after this step
+                                 (tau + 1 >= frames + S - 1), else 0                               */
 } cfgms_step_args;
+
+#define CFGMS_FRAMES_UNSET 2147483647 /* n_frames value meaning "no frame count yet" (no drain)   */
 
 /*
  * cfgms_step — steps 1-4 above for one batch.  Every pointer in `args` is a DEVICE pointer.
@@ -143,7 +157,8 @@ int cfgms_step(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stream);
 /*
  * cfgms_step_host — same step with HOST buffers: hidden, pair_map, w, temp, top_k, step,
  * req_id, n_frames, force_token, tokens_out, frame_out and frame_index_out are HOST pointers
- * (pinned memory recommended); `delayed` and `logits_out` stay DEVICE pointers (per-request state lives in HBM) or NULL.  Copies the
+ * (pinned memory recommended); `delayed`, `logits_out` and the request-state outputs (`step_next_out`,
+ * `n_frames_next_out`, `done_out`) stay DEVICE pointers (per-request state lives in HBM) or NULL.  Copies the
  * inputs host->device, runs the step, copies tokens_out device->host and synchronises the
  * stream.  Bytes moved per call are reported by cfgms_get_info.
  */

@@ -284,7 +284,7 @@ int oracle_step_ex(const uint16_t* heads, const uint16_t* embeds, const uint16_t
         uint32_t rid = req_id ? req_id[c] : (uint32_t)c;
         int32_t tok, flags = 0;
         double margin = INFINITY;
-        int active = (i <= tau) && (n_frames == NULL || tau < n_frames[c] + i);      /* O5 */
+        int active = (i <= tau) && (n_frames == NULL || tau - i < n_frames[c]);      /* O5: tau < F + i, written without the sum so that F = INT32_MAX ("no frame count yet", C27) cannot overflow */
         if (!active) {
             tok = pad_token;
             flags = ORC_INACTIVE;

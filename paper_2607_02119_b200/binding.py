@@ -19,6 +19,7 @@ CFGMS_CFG_SINGLE_CTA = 4
 CFGMS_CFG_CTA_PAIR = 8
 CFGMS_CFG_NO_OVERLAP = 16
 CFGMS_CFG_OVERLAP = 32
+CFGMS_FRAMES_UNSET = 2 ** 31 - 1
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
           5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
@@ -46,7 +47,8 @@ class cfgms_step_args(C.Structure):
                 ("seed", C.c_uint64), ("step", C.c_void_p), ("req_id", C.c_void_p), ("n_frames", C.c_void_p),
                 ("tokens_out", C.c_void_p), ("delayed", C.c_void_p), ("T_cap", C.c_int32),
                 ("logits_out", C.c_void_p), ("force_token", C.c_void_p), ("frame_out", C.c_void_p),
-                ("frame_index_out", C.c_void_p)]
+                ("frame_index_out", C.c_void_p), ("eos_token", C.c_int32), ("step_next_out", C.c_void_p),
+                ("n_frames_next_out", C.c_void_p), ("done_out", C.c_void_p)]
 
 
 class cfgms_info(C.Structure):
@@ -185,7 +187,8 @@ class Context:
             pass
 
     def _args(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
-              logits_out, dev: str, force_token=None, frame_out=None, frame_index_out=None) -> cfgms_step_args:
+              logits_out, dev: str, force_token=None, frame_out=None, frame_index_out=None, eos_token=-1,
+              step_next_out=None, n_frames_next_out=None, done_out=None) -> cfgms_step_args:
         R = int(hidden.shape[0])
         _check(hidden, "hidden", (torch.bfloat16, torch.float32), dev, R * self.d)
         if hidden.dim() != 2 or hidden.shape[1] != self.d:
@@ -219,14 +222,19 @@ class Context:
         _check(frame_out, "frame_out", torch.int32, dev, R * self.S, optional=True)
         _check(frame_index_out, "frame_index_out", torch.int32, dev, R, optional=True)
         a.force_token, a.frame_out, a.frame_index_out = _ptr(force_token), _ptr(frame_out), _ptr(frame_index_out)
+        for t, name in ((step_next_out, "step_next_out"), (n_frames_next_out, "n_frames_next_out"), (done_out, "done_out")):
+            _check(t, name, torch.int32, "cuda", R, optional=True)
+        a.eos_token = int(eos_token)
+        a.step_next_out, a.n_frames_next_out, a.done_out = _ptr(step_next_out), _ptr(n_frames_next_out), _ptr(done_out)
         return a
 
     def step(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
              delayed=None, logits_out=None, stream=None, force_token=None, frame_out=None,
-             frame_index_out=None) -> None:
+             frame_index_out=None, eos_token=-1, step_next_out=None, n_frames_next_out=None, done_out=None) -> None:
         """cfgms_step: device tensors, enqueue only."""
         a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
-                       logits_out, "cuda", force_token, frame_out, frame_index_out)
+                       logits_out, "cuda", force_token, frame_out, frame_index_out, eos_token, step_next_out,
+                       n_frames_next_out, done_out)
         rc = _lib().cfgms_step(self._h, C.byref(a), _stream_ptr(stream))
         if rc != 0:
             raise CfgmsError(rc, "cfgms_step")

@@ -388,6 +388,8 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.tokens_out = a->tokens_out; fp.delayed = a->delayed; fp.T_cap = a->T_cap;
     fp.cand_val = c->cand_val; fp.cand_src = c->cand_src;
     fp.force_token = a->force_token; fp.frame_out = a->frame_out; fp.frame_index_out = a->frame_index_out;
+    fp.eos_token = a->eos_token; fp.step_next_out = a->step_next_out; fp.n_frames_next_out = a->n_frames_next_out;
+    fp.done_out = a->done_out;
     fp.ready = gp.ready;
     fp.done = overlap ? c->ready + (c->ready_words - 33) : nullptr;
     fp.stats = overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 32)) : nullptr;

@@ -46,6 +46,10 @@ struct FinalizeParams {
     const int32_t* force_token;  // [R][S]
     int32_t* frame_out;          // [R][S]
     int32_t* frame_index_out;    // [R]
+    int32_t eos_token;           // device-resident request state (include/cfgms.h): end-of-audio id, < 0 = none
+    int32_t* step_next_out;      // [R]
+    int32_t* n_frames_next_out;  // [R]
+    int32_t* done_out;           // [R]
     int* ready;               // nullable [S][num_row_blocks]
     int* done;                // CTAs of this grid that finished; the last one clears ready[] for the next step
     unsigned long long* stats;// [16] cells that arrived before their group was complete (summed on the host)
@@ -115,6 +119,17 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
     if (p.delayed) {
         const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
         p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
+    }
+    if (i == 0 && (p.step_next_out || p.n_frames_next_out || p.done_out)) {
+        // request state for the next step, by the thread of the PRIMARY stream's cell: the
+        // frame count is fixed the moment stream 0 emits the end-of-audio token; other streams of this
+        // step are unaffected (tau < tau + i), so nothing in this launch depends on what is written here
+        constexpr int kUnset = 2147483647;
+        int F = p.n_frames ? p.n_frames[r] : kUnset;
+        if (F == kUnset && p.eos_token >= 0 && token == p.eos_token) F = tau;
+        if (p.step_next_out) p.step_next_out[r] = tau + 1;
+        if (p.n_frames_next_out) p.n_frames_next_out[r] = F;
+        if (p.done_out) p.done_out[r] = (F != kUnset && tau + 1 >= F + p.S - 1) ? 1 : 0;
     }
     if (i == p.S - 1 && (p.frame_out || p.frame_index_out)) {
         const int f = tau - p.S + 1;

@@ -193,3 +193,61 @@ def test_feedback_is_the_correctly_rounded_sum(dev, shape):
     assert np.all(np.abs(got - want) <= tol), float(np.max(np.abs(got - want) / _bf16_ulp(want)))
     assert np.array_equal(got[1][: d], got[0][: d]) if R >= 2 else True
     ctx.close()
+
+
+# ------------------------------------------------------------------ W4
+def test_device_resident_state_drives_requests_through_drain(dev):
+    """Self-driving decode loop: step / frame-count state ping-pongs between two device buffers, the
+    end-of-audio token on stream 0 (injected per request at a different step through force_token) fixes
+    the frame count, drain follows, done flags rise; frame emission (W1) hands out exactly F frames.
+    Every step is compared with the oracle driven by oracle.advance_state on the host."""
+    wl = _custom(pairs=3, singles=2, d=128, S=4, V=256, T=40, mixed=True)
+    wl.temp[:] = 0.0                       # greedy: no close ties to excuse, tokens must match exactly
+    dw = DeviceWorkload(wl, dev, T_cap=wl.S)
+    R, S, EOS = wl.R, wl.S, wl.V - 1
+    heads = [int(c) for c in wl.head_rows()]
+    eos_at = {c: 3 + 4 * k for k, c in enumerate(heads)}
+    eos_at[heads[-1]] = 10 ** 6            # the last request never ends inside the window
+    UNSET = oracle.F_UNSET
+    st = [torch.zeros(R, dtype=torch.int32, device=dev), torch.zeros(R, dtype=torch.int32, device=dev)]
+    nf = [torch.full((R,), UNSET, dtype=torch.int32, device=dev), torch.full((R,), UNSET, dtype=torch.int32, device=dev)]
+    done = torch.zeros(R, dtype=torch.int32, device=dev)
+    frame = torch.zeros((R, S), dtype=torch.int32, device=dev)
+    fidx = torch.zeros(R, dtype=torch.int32, device=dev)
+    o_tau = {c: 0 for c in heads}
+    o_F = {c: UNSET for c in heads}
+    n_frames_emitted = {c: 0 for c in heads}
+    for t in range(30):
+        ft = np.full((R, S), -1, dtype=np.int32)
+        for c in heads:
+            if o_tau[c] == eos_at[c]:
+                ft[c, 0] = EOS
+        a, b = st[t & 1], st[(t + 1) & 1]
+        fa, fb = nf[t & 1], nf[(t + 1) & 1]
+        dw.ctx.step(dw.hidden(t), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, a, dw.tokens, req_id=dw.req_id,
+                    n_frames=fa, delayed=dw.delayed, force_token=torch.from_numpy(ft).to(dev), frame_out=frame,
+                    frame_index_out=fidx, eos_token=EOS, step_next_out=b, n_frames_next_out=fb, done_out=done)
+        dw.check_no_device_error()
+        # the oracle, driven by its own state
+        o_step = np.zeros(R, dtype=np.int32)
+        o_nf = np.full(R, UNSET, dtype=np.int32)
+        for c in heads:
+            o_step[c], o_nf[c] = o_tau[c], o_F[c]
+        ref = oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, o_step,
+                          wl.req_id, o_nf, wl.pad_token, force_token=ft)
+        got = dw.tokens.cpu().numpy()
+        tok0 = {}
+        for j, (c, i) in enumerate(ref.cells):
+            assert got[c, i] == ref.tok[j], (t, c, i)
+            if i == 0:
+                tok0[int(c)] = int(ref.tok[j])
+        g_step, g_nf, g_done, g_fidx = b.cpu().numpy(), fb.cpu().numpy(), done.cpu().numpy(), fidx.cpu().numpy()
+        for c in heads:
+            o_tau[c], o_F[c], d = oracle.advance_state(o_tau[c], o_F[c], tok0[c], EOS, S)
+            assert (g_step[c], g_nf[c], bool(g_done[c])) == (o_tau[c], o_F[c], d), (t, c)
+            if g_fidx[c] >= 0:
+                assert g_fidx[c] == n_frames_emitted[c]        # frames come out in order, none twice
+                n_frames_emitted[c] += 1
+    for c in heads[:-1]:
+        assert o_F[c] == eos_at[c] and n_frames_emitted[c] == o_F[c]      # exactly F frames were handed out
+    assert o_F[heads[-1]] == UNSET
