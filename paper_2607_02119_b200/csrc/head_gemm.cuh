@@ -19,15 +19,15 @@
 // shared-memory fill and read traffic of the row operand (the limiter of the one-CTA kernel at
 // large batches).  Each CTA's epilogue reads its own 128 accumulator lanes from its own TMEM.
 //
-// Warp roles (320 threads, persistent over tiles, 1 CTA/SM):
-//   warp 0      TMA producer: W tile [128 x 64] + H tile [BN (or BN/2) x 64] bf16 -> 128B-swizzled ring
+// Warp roles (352 threads, persistent over tiles, 1 CTA/SM):
+//   warp 0, 2   TMA producers: warp 0 the W tile [128 x 64], warp 2 the H tile [BN (or BN/2) x 64] bf16 -> 128B-swizzled ring
 //   warp 1      TMEM allocator + single-thread tcgen05.mma issuer (leader CTA only when kPair),
 //               2 accumulator stages in TMEM so the epilogue of tile t overlaps the mainloop of t+1
-//   warps 2-9   epilogue, two warps per TMEM lane quarter (alternate 64-column slab pairs):
+//   warps 3-10  epilogue, two warps per TMEM lane quarter (alternate 64-column slab pairs):
 //               tcgen05.ld -> merge -> x 1/temp -> z spill (fp32) -> per-chunk top-4 candidates
 //
 // Register budget: the register file is split over the SM's four sub-partitions (16 K registers
-// each) and the ten warps land 3/3/2/2 on them.  At 168 registers per thread a three-warp
+// each) and the eleven warps land 3/3/3/2 on them.  At 168 registers per thread a three-warp
 // sub-partition is full (16128 of 16384), so NO warp of any other grid can become resident on the
 // SM (measured: even a 32-thread kernel waits for this one to exit; setmaxnreg.dec does not help,
 // it returns registers to the CTA's own pool only).  Capped at 152, every sub-partition keeps
@@ -43,7 +43,7 @@ constexpr int kBM = 128;        // vocabulary rows per CTA tile (UMMA M, or half
 constexpr int kBK = 64;         // K elements per stage (128 B = swizzle span)
 constexpr int kMaxBN = 256;     // batch rows per tile (UMMA N)
 constexpr int kEpiWarps = 8;
-constexpr int kCtrlWarps = 2;     // TMA producer, MMA issuer
+constexpr int kCtrlWarps = 3;     // TMA producer (weights), MMA issuer, TMA producer (hidden rows)
 constexpr int kGemmMaxRegs = 152; // see "Register budget" above
 constexpr int kGemmThreads = 32 * (kCtrlWarps + kEpiWarps);
 constexpr int kMaxStages = 8;
@@ -216,10 +216,14 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     // block) groups through p.ready while the GEMM is still running.
     pdl_launch_dependents();
 
-    if (warp == 0) {
-        // ================= TMA producer (every CTA) =================
+    if (warp == 0 || warp == 2) {
+        // ================= TMA producers (every CTA): warp 0 loads the weight tiles, warp 2 the row tiles ====
+        // Two issuing warps because one thread's TMA issue rate caps the SM's intake (probe: 16 KB boxes
+        // from one / two / four issuing warps of a CTA reach 17 / 33 / 58 B/clk/SM out of L2).
         // The whole warp walks the loop (warp-uniform state stays in uniform registers); one
-        // elected lane issues.  Transaction bytes of both CTAs land on the leader's barrier.
+        // elected lane issues.  Transaction bytes of both CTAs land on the leader's barrier; the
+        // weight producer of the leader posts the expected byte count of the whole stage.
+        const bool load_w = warp == 0;
         const uint32_t full_sig = kPair ? mapa_shared(bar_full, 0u) : bar_full;
         const uint32_t tx_bytes = (a_bytes + b_bytes) * (kPair ? 2u : 1u);
         int s = 0;
@@ -232,13 +236,13 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             for (int kb = 0; kb < p.num_kb; ++kb) {
                 mbar_wait(bar_empty + 8 * s, phase ^ 1, p.err, 1);
                 if (elect_one()) {
-                    if (leader) mbar_arrive_expect_tx(bar_full + 8 * s, tx_bytes);
-                    if (kPair) {
-                        tma_load_2d_pair(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
-                        tma_load_2d_pair(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
+                    if (load_w) {
+                        if (leader) mbar_arrive_expect_tx(bar_full + 8 * s, tx_bytes);
+                        if (kPair) tma_load_2d_pair(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
+                        else tma_load_2d(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
                     } else {
-                        tma_load_2d(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
-                        tma_load_2d(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
+                        if (kPair) tma_load_2d_pair(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
+                        else tma_load_2d(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
                     }
                 }
                 __syncwarp();
@@ -286,7 +290,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             }
         }
     } else {
-        // ================= epilogue (warps 2..9, every CTA) =================
+        // ================= epilogue (warps 3..10, every CTA) =================
         const int ew = warp - kCtrlWarps;
         const int quarter = warp & 3;             // TMEM lane quarter this warp may read
         const int half = ew >> 2;                 // which slab pairs (alternating) this warp takes
