@@ -344,6 +344,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
                          (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
     gp.ready = overlap ? c->ready : nullptr;
     gp.V = c->V;
+    gp.split_tma = gp.num_tiles < kOverlapMinWaves * workers ? 1 : 0;
     // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;

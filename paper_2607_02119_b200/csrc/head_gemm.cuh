@@ -75,6 +75,7 @@ struct GemmParams {
     int* err;            // sticky error word {code | row << 8}
     int* ready;          // nullable [S][num_row_blocks]: epilogue-warp arrivals per (stream, row block), see K2
     int V;               // tokens per stream (ready != nullptr requires V % kBM == 0)
+    int split_tma;       // 1: warp 2 issues the row-tile loads; 0: warp 0 issues both (warp 2 idles)
     uint64_t policy_w, policy_h;
 };
 
@@ -216,14 +217,18 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     // block) groups through p.ready while the GEMM is still running.
     pdl_launch_dependents();
 
-    if (warp == 0 || warp == 2) {
+    if (warp == 2 && !p.split_tma) {
+        // idle: warp 0 issues both loads (see below); wait at the teardown barrier
+    } else if (warp == 0 || warp == 2) {
         // ================= TMA producers (every CTA): warp 0 loads the weight tiles, warp 2 the row tiles ====
-        // Two issuing warps because one thread's TMA issue rate caps the SM's intake (probe: 16 KB boxes
-        // from one / two / four issuing warps of a CTA reach 17 / 33 / 58 B/clk/SM out of L2).
+        // Two issuing warps where the GEMM is short (one or two waves: configs 2-4 gain 3-5 %); a long,
+        // power-capped GEMM (config 5) measured ~3 % slower with the extra spinning warp, so there warp 0
+        // issues both loads and warp 2 idles (p.split_tma).
         // The whole warp walks the loop (warp-uniform state stays in uniform registers); one
         // elected lane issues.  Transaction bytes of both CTAs land on the leader's barrier; the
         // weight producer of the leader posts the expected byte count of the whole stage.
         const bool load_w = warp == 0;
+        const bool load_h = warp == 2 || !p.split_tma;
         const uint32_t full_sig = kPair ? mapa_shared(bar_full, 0u) : bar_full;
         const uint32_t tx_bytes = (a_bytes + b_bytes) * (kPair ? 2u : 1u);
         int s = 0;
@@ -240,7 +245,8 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                         if (leader) mbar_arrive_expect_tx(bar_full + 8 * s, tx_bytes);
                         if (kPair) tma_load_2d_pair(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
                         else tma_load_2d(smem_a + s * a_bytes, &tmap_w, full_sig + 8 * s, kb * kBK, vt * kBM, p.policy_w);
-                    } else {
+                    }
+                    if (load_h) {
                         if (kPair) tma_load_2d_pair(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
                         else tma_load_2d(smem_b + s * b_bytes, &tmap_h, full_sig + 8 * s, kb * kBK, row0, p.policy_h);
                     }
