@@ -28,7 +28,7 @@ METRIC = "cfg_audio_frames_per_sec"
 UNIT = "frames/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per head-GEMM launch from the committed
 # `ncu --set full` capture (profiles/), keyed by config; None until captured.
-NCU_TRAFFIC_BYTES = {5: 348.52e6}   # profiles/r1c_ncu_full_config5.md: dram read + written per head-GEMM launch
+NCU_TRAFFIC_BYTES = {5: 345.55e6}   # profiles/r1c_ncu_full_config5.md: dram read + written per head-GEMM launch
 
 
 def load_peaks():
@@ -60,8 +60,9 @@ class ClockSampler:
 
     def _run(self):
         nv = self.nv
-        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
-                 0x80: "hw_power_brake_slowdown"}
+        names = {0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x10: "sync_boost",
+                 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+                 0x100: "display_clock_setting"}
         while not self._stop.is_set():
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
@@ -74,7 +75,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.005)
+            time.sleep(0.002)
 
     def __enter__(self):
         if self.nv is not None:
