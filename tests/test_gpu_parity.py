@@ -360,3 +360,47 @@ def test_overlap_counters_survive_steps_whose_cells_are_mostly_pad(dev):
             assert torch.equal(ov.tokens, ser.tokens), (rep, t)
     assert ov.ctx.info()["overlap"] == 1
     ov.check_no_device_error()
+
+
+@pytest.mark.parametrize("cfg,n_cells", [(5, 96), (3, 64), (2, 256)])
+def test_bench_launch_configuration_graph_replay(dev, cfg, n_cells):
+    """The launch configuration bench.py times: default policy (config 5: lean GEMM + dependent finalize
+    beside it; configs 2-3: full-register GEMM, serial finalize), no debug tap, consecutive steps
+    captured in ONE CUDA graph and replayed.  Tokens of every captured step are read back from the
+    delayed buffer and compared with the oracle on a seeded sample of cells."""
+    wl = workloads.make_config(cfg)
+    dw = DeviceWorkload(wl, dev)
+    steps = [0, wl.S - 1, wl.S + 2, 40, 41, 42]
+    st = {t: wl.step(t).to(dev) for t in steps}
+    run = lambda t: dw.ctx.step(dw.hidden(t), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, st[t], dw.tokens,
+                                req_id=dw.req_id, n_frames=dw.n_frames, delayed=dw.delayed)
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        run(steps[0])
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g, stream=s):
+        for t in steps:
+            run(t)
+    dw.delayed.fill_(-1)
+    g.replay()
+    g.replay()
+    dw.check_no_device_error()
+    assert dw.ctx.info()["overlap"] == (1 if cfg == 5 else 0)
+    delayed = dw.delayed.cpu().numpy()
+    n_close = n_mismatch = 0
+    for n, t in enumerate(steps):
+        cells = sample_cells(wl, n_cells, seed=900 + n)
+        ref = oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, wl.step(t),
+                          wl.req_id, wl.n_frames, wl.pad_token, cells=cells, hidden_is_f32=wl.hidden_f32)
+        tau = wl.step(t).numpy()
+        for j, (c, i) in enumerate(ref.cells):
+            got = delayed[c, int(tau[c]) % dw.T_cap, i]
+            if ref.flags[j] & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
+                n_close += 1
+                n_mismatch += int(got != ref.tok[j])
+            else:
+                assert got == ref.tok[j], (t, c, i, got, ref.tok[j], ref.margin[j])
+    print(f"config{cfg} graph replay: close ties {n_close}, of which differ {n_mismatch}")
