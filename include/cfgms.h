@@ -71,7 +71,14 @@ typedef struct {
     int32_t row_tile;  /* debug/tuning: batch rows per accumulator tile (multiple of 64,
                           <= 256); 0 = chosen from R and the SM count                           */
     int32_t max_stages; /* debug/tuning: cap on the head GEMM's TMA ring depth (0 = as deep as fits)   */
-    int32_t reserved[3];
+    int32_t stream_base;   /* stream-sharded heads (one context per GPU, each holding some of the     */
+    int32_t stream_stride; /* streams): local stream i of THIS context is global stream
+                              stream_base + i * stream_stride.  The delay pattern, the noise key and
+                              the primary-stream rules use the global index, so the shards together
+                              sample exactly what one unsharded context samples; the caller gathers
+                              tokens_out [R][S_local] of all shards (<= 32 KB per step).  stride <= 0
+                              means unsharded (base 0, stride 1).  frame_out needs an unsharded context */
+    int32_t reserved[1];
 } cfgms_config;
 
 /*

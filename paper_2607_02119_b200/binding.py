@@ -38,7 +38,8 @@ class CfgmsError(RuntimeError):
 
 class cfgms_config(C.Structure):
     _fields_ = [("max_rows", C.c_int32), ("pad_token", C.c_int32), ("flags", C.c_uint32),
-                ("row_tile", C.c_int32), ("max_stages", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("row_tile", C.c_int32), ("max_stages", C.c_int32), ("stream_base", C.c_int32),
+                ("stream_stride", C.c_int32), ("reserved", C.c_int32 * 1)]
 
 
 class cfgms_step_args(C.Structure):
@@ -143,7 +144,7 @@ class Context:
     def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
                  cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0,
-                 force_overlap: bool = False):
+                 force_overlap: bool = False, stream_base: int = 0, stream_stride: int = 0):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -154,6 +155,7 @@ class Context:
         cfg.max_rows = int(max_rows)
         cfg.row_tile = int(row_tile)
         cfg.max_stages = int(max_stages)
+        cfg.stream_base, cfg.stream_stride = int(stream_base), int(stream_stride)   # stream-sharded heads
         if pad_token is not None:
             cfg.pad_token = int(pad_token)
             cfg.flags |= CFGMS_CFG_PAD_TOKEN

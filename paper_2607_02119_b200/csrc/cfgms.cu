@@ -43,6 +43,7 @@ struct cfgms_ctx {
     int S = 0, d = 0, V = 0, NT = 0;
     int device = 0, num_sms = 0;
     int max_rows = 0, pad_token = 0, row_tile_override = 0, max_stages = 0;
+    int stream_base = 0, stream_stride = 1;   // stream-sharded heads: global stream of local stream i
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT] what the epilogue adds: bias_base (+ the caller's logit bias)
@@ -128,6 +129,7 @@ int validate_step(const cfgms_ctx* c, const cfgms_step_args* a) {
     if (a->R > c->max_rows) return CFGMS_ERR_SHAPE;
     if (a->delayed && a->T_cap < 1) return CFGMS_ERR_ARG;
     if ((a->frame_out || a->frame_index_out) && (!a->delayed || a->T_cap < c->S)) return CFGMS_ERR_ARG;
+    if ((a->frame_out || a->frame_index_out) && (c->stream_base != 0 || c->stream_stride != 1)) return CFGMS_ERR_ARG;   // a frame needs every stream
     return CFGMS_OK;
 }
 
@@ -176,6 +178,8 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     c->pad_token = (cfg && (cfg->flags & CFGMS_CFG_PAD_TOKEN)) ? cfg->pad_token : V;
     c->row_tile_override = cfg ? cfg->row_tile : 0;
     c->max_stages = (cfg && cfg->max_stages >= 2) ? cfg->max_stages : kMaxStages;
+    if (cfg && cfg->stream_stride > 0) { c->stream_base = cfg->stream_base; c->stream_stride = cfg->stream_stride; }
+    if (c->stream_base < 0) { delete c; return CFGMS_ERR_ARG; }
     c->pair_mode = (cfg && (cfg->flags & CFGMS_CFG_SINGLE_CTA)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_CTA_PAIR)) ? 2 : 0;
     if (c->row_tile_override < 0 || c->row_tile_override > kMaxBN || (c->row_tile_override % 64) != 0) {
         delete c;
@@ -396,6 +400,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.stats = overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 32)) : nullptr;
     fp.err = c->err;
     fp.BN = BN; fp.num_row_blocks = nrb;
+    fp.stream_base = c->stream_base; fp.stream_stride = c->stream_stride;
     fp.ready_target = (c->V / kBM) * kEpiWarps;   // every epilogue warp of every vocabulary tile of the stream
     if (c->use_cand) {
         const size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;

@@ -55,6 +55,7 @@ struct FinalizeParams {
     unsigned long long* stats;// [16] cells that arrived before their group was complete (summed on the host)
     int* err;                 // sticky error word
     int BN, num_row_blocks, ready_target;
+    int stream_base, stream_stride;   // global stream of local stream i = base + i * stride (stream-sharded heads)
 };
 
 // Philox4x32-10 (Salmon et al. 2011): ten rounds of two 32x32->64 multiplies with key bumps.
@@ -104,6 +105,10 @@ __device__ __forceinline__ uint32_t float_key_fast(float f) {
     return u ^ (static_cast<uint32_t>(static_cast<int32_t>(u) >> 31) | 0x80000000u);
 }
 
+// Stream-sharded heads (W5): this context may hold only the streams
+// {base + i * stride}; the delay pattern, the noise key and the primary-stream rules use the GLOBAL index.
+__device__ __forceinline__ int global_stream(const FinalizeParams& p, int i) { return p.stream_base + i * p.stream_stride; }
+
 // Token of an ACTIVE cell given by the caller (phase machine hook), or -1.
 __device__ __forceinline__ int forced_token(const FinalizeParams& p, int r, int i) {
     return p.force_token ? p.force_token[static_cast<size_t>(r) * p.S + i] : -1;
@@ -120,7 +125,7 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
         const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
         p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
     }
-    if (i == 0 && (p.step_next_out || p.n_frames_next_out || p.done_out)) {
+    if (global_stream(p, i) == 0 && (p.step_next_out || p.n_frames_next_out || p.done_out)) {
         // request state for the next step, by the thread of the PRIMARY stream's cell: the
         // frame count is fixed the moment stream 0 emits the end-of-audio token; other streams of this
         // step are unaffected (tau < tau + i), so nothing in this launch depends on what is written here
@@ -245,7 +250,8 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
     if (pm >= 0 && (r & 1)) return;  // companion row: its cond row writes both
 
     const int tau = p.step[r];
-    bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    const int gi = global_stream(p, i);
+    bool active = (gi <= tau) && (p.n_frames == nullptr || tau - gi < p.n_frames[r]);
     int token = p.pad_token;
     if (active) {
         const int ft = forced_token(p, r, i);
@@ -322,7 +328,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
                 const uint32_t ck = cand_key[e];
                 if (ck >= thr_key) {
                     const int v = cand_idx[e];
-                    best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                    best_update(best, key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
                 }
             }
         } else {
@@ -332,7 +338,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
                 const int v = j * kFinThreads + tid;
                 if (v < V) {
                     float s = key_float(key[j]);
-                    if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v);
+                    if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v);
                     best_update(best, s, v);
                 }
             }
@@ -355,7 +361,8 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
     const int pm = p.pair_map[r];
     if (pm >= 0 && (r & 1)) return;
     const int tau = p.step[r];
-    bool active = (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    const int gi = global_stream(p, i);
+    bool active = (gi <= tau) && (p.n_frames == nullptr || tau - gi < p.n_frames[r]);
     int token = p.pad_token;
     if (active) {
         const int ft = forced_token(p, r, i);
@@ -384,7 +391,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
             const uint32_t k = dyn[v];
             if (k >= thr_key) {
                 float s = key_float(k);
-                if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v);
+                if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v);
                 best_update(best, s, v);
             }
         }
@@ -454,7 +461,8 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     int* list_v = reinterpret_cast<int*>(list_key + cap);
 
     const int tau = p.step[r];
-    bool active = valid && (i <= tau) && (p.n_frames == nullptr || tau - i < p.n_frames[r]);
+    const int gi = global_stream(p, i);
+    bool active = valid && (gi <= tau) && (p.n_frames == nullptr || tau - gi < p.n_frames[r]);
     int token = p.pad_token;
     if (active) {
         const int ft = forced_token(p, r, i);
@@ -664,7 +672,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                         const uint32_t ck = list_key[e];
                         if (ck >= thr) {
                             const int v = list_v[e];
-                            best_update(best, greedy ? key_float(ck) : key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                            best_update(best, greedy ? key_float(ck) : key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
                         }
                     }
                 } else {
@@ -672,7 +680,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     for (int v = lane; v < V; v += 32) {
                         const float zv = __ldcg(zr + v);
                         if (float_key(zv) >= thr_full)
-                            best_update(best, greedy ? zv + 0.0f : zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                            best_update(best, greedy ? zv + 0.0f : zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
                     }
                 }
             }
@@ -683,7 +691,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
             for (int v = lane; v < V; v += 32) {
                 const float zv = __ldcg(zr + v);
                 if (float_key(zv) >= thr_full)
-                    best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, i, v), v);
+                    best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
             }
         }
         best = warp_argmax(best);

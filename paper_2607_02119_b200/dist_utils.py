@@ -67,3 +67,41 @@ def whole_job_rate(units_this_rank: float, elapsed_ms_this_rank: float, device=N
     total = sum_over_ranks(units_this_rank, device)
     worst = max_over_ranks(elapsed_ms_this_rank, device)
     return total / (worst * 1e-3), worst
+
+
+# ---------------------------------------------------------------- stream-sharded heads (W5)
+# The alternative sharding for the weight-streaming regime: GPU g holds the head slices of the streams
+# {g, g + G, g + 2G, ...} (cfgms_config.stream_base = g, stream_stride = G), every GPU sees all rows, and the
+# only exchange per step is an all-gather of n_rows x S_local int32 tokens (<= 32 KB).
+
+def stream_shard(rank: int, world: int, S: int) -> Tuple[int, int, int]:
+    """-> (stream_base, stream_stride, S_local) of this rank: streams rank, rank + world, ..."""
+    if not (0 <= rank < world) or S < world:
+        raise ValueError("need 0 <= rank < world <= S")
+    return rank, world, len(range(rank, S, world))
+
+
+def merge_stream_shards(shards, S: int) -> torch.Tensor:
+    """shards[g]: int32 [R][S_local(g)] tokens of rank g (columns = its local streams) -> [R][S]."""
+    world = len(shards)
+    R = shards[0].shape[0]
+    out = torch.empty((R, S), dtype=shards[0].dtype, device=shards[0].device)
+    for g, t in enumerate(shards):
+        cols = list(range(g, S, world))
+        out[:, cols] = t[:, :len(cols)]
+    return out
+
+
+def all_gather_stream_tokens(tokens_local: torch.Tensor, S: int) -> torch.Tensor:
+    """The step's one exchange: every rank contributes its [R][S_local] tokens and receives [R][S].
+    Ranks with fewer local streams pad to the widest shard (S need not divide the world size)."""
+    if not dist.is_initialized():
+        return merge_stream_shards([tokens_local], S)
+    world, rank = dist.get_world_size(), dist.get_rank()
+    widest = len(range(0, S, world))
+    R = tokens_local.shape[0]
+    mine = torch.full((R, widest), -1, dtype=tokens_local.dtype, device=tokens_local.device)
+    mine[:, :tokens_local.shape[1]] = tokens_local
+    parts = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(parts, mine)
+    return merge_stream_shards(parts, S)

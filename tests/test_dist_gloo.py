@@ -39,6 +39,31 @@ def test_two_rank_sharding_and_max_over_ranks():
         assert abs(rate - (2 * 512 * 100.0) / 0.025) < 1e-6
 
 
+def _shard_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    from paper_2607_02119_b200 import dist_utils
+    dist_utils.init("gloo")
+    S, R = 9, 6                                    # 9 streams over 2 ranks: 5 + 4 local streams
+    base, stride, s_local = dist_utils.stream_shard(rank, world, S)
+    full = torch.arange(R * S, dtype=torch.int32).reshape(R, S)      # what an unsharded head would emit
+    mine = full[:, base::stride].contiguous()
+    assert mine.shape == (R, s_local)
+    out[rank] = (base, stride, s_local, dist_utils.all_gather_stream_tokens(mine, S).tolist())
+    dist.destroy_process_group()
+
+
+def test_two_rank_stream_sharded_token_all_gather():
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_shard_worker, args=(world, 29613, out), nprocs=world, join=True)
+    full = torch.arange(6 * 9, dtype=torch.int32).reshape(6, 9).tolist()
+    assert out[0][:3] == (0, 2, 5) and out[1][:3] == (1, 2, 4)
+    assert out[0][3] == full and out[1][3] == full
+
+
 def test_single_process_is_identity():
     sys.path.insert(0, ROOT)
     from paper_2607_02119_b200 import dist_utils

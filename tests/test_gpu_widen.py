@@ -251,3 +251,43 @@ def test_device_resident_state_drives_requests_through_drain(dev):
     for c in heads[:-1]:
         assert o_F[c] == eos_at[c] and n_frames_emitted[c] == o_F[c]      # exactly F frames were handed out
     assert o_F[heads[-1]] == UNSET
+
+
+# ------------------------------------------------------------------ W5: stream-sharded heads
+@pytest.mark.parametrize("world", [2, 3])
+def test_stream_sharded_contexts_sample_what_the_unsharded_head_samples(dev, world):
+    """Each 'rank' (here: independent contexts on one GPU, launched one after the other — no kernel waits
+    on another) holds the head slices of streams {g, g + G, ...} with stream_base / stream_stride;
+    merged, their tokens must equal the unsharded context's bit for bit (counter-based noise keyed by
+    the GLOBAL stream, delay pattern on the global stream index), PAD cells included."""
+    import paper_2607_02119_b200 as pkg
+    from paper_2607_02119_b200 import dist_utils
+    wl = _custom(pairs=5, singles=2, d=256, S=9, V=256, T=24, mixed=True)       # OpusLM-like 9 streams
+    full = DeviceWorkload(wl, dev)
+    R, S = wl.R, wl.S
+    shards = []
+    for g in range(world):
+        base, stride, s_local = dist_utils.stream_shard(g, world, S)
+        heads = wl.heads[base::stride].contiguous().to(dev)
+        embeds = wl.embeds[base::stride].contiguous().to(dev)
+        assert heads.shape[0] == s_local
+        ctx = pkg.Context(heads, embeds, max_rows=R, stream_base=base, stream_stride=stride)
+        shards.append((ctx, heads, embeds, torch.full((R, s_local), -1, dtype=torch.int32, device=dev)))
+    for t in (0, 1, 4, 8, 9, 15, 23):
+        full.step(t)
+        st = wl.step(t).to(dev)
+        for ctx, _, _, tok in shards:
+            ctx.step(full.hidden(t), full.pair_map, full.w, full.temp, full.top_k, wl.seed, st, tok,
+                     req_id=full.req_id, n_frames=full.n_frames)
+        torch.cuda.synchronize()
+        merged = dist_utils.merge_stream_shards([s[3] for s in shards], S)
+        assert torch.equal(merged, full.tokens), t
+    # a frame needs every stream: sharded contexts refuse frame emission
+    fr = torch.zeros((R, shards[1][3].shape[1]), dtype=torch.int32, device=dev)
+    dl = torch.zeros((R, 16, shards[1][3].shape[1]), dtype=torch.int32, device=dev)
+    with pytest.raises(pkg.CfgmsError) as e:
+        shards[1][0].step(full.hidden(0), full.pair_map, full.w, full.temp, full.top_k, wl.seed, wl.step(0).to(dev),
+                          shards[1][3], delayed=dl, frame_out=fr)
+    assert e.value.status == 1      # CFGMS_ERR_ARG
+    for ctx, *_ in shards:
+        ctx.close()
