@@ -344,8 +344,9 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     // Overlap K2 with K1 only where finished groups appear long before the GEMM ends (several waves of
     // tiles): a one- or two-wave GEMM has nothing to hide behind, and the lean register budget and
     // the polling finalize warps then cost more than the early launch saves (measured).
-    const bool overlap = c->overlap && !prof &&
-                         (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
+    // (While the profiling events are recorded the SAME kernels run, but K2 is launched strictly after K1 so
+    // that each has a duration of its own.)
+    const bool overlap = c->overlap && (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
     gp.ready = overlap ? c->ready : nullptr;
     gp.V = c->V;
     gp.split_tma = gp.num_tiles < kOverlapMinWaves * workers ? 1 : 0;
@@ -404,7 +405,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.ready_target = (c->V / kBM) * kEpiWarps;   // every epilogue warp of every vocabulary tile of the stream
     if (c->use_cand) {
         const size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;
-        const int cells = a->R * c->S;
+        const int cells = 2 * ((a->R + 1) / 2) * c->S;   // (stream, even rows | odd rows): see the kernel's cell order
         const int fblocks = (cells + kCandWarps - 1) / kCandWarps;
         using FinFn = void (*)(const FinalizeParams);
         const FinFn ffn = c->V <= 1024 ? cfgms_finalize_cand_kernel<1> : c->V <= 2048 ? cfgms_finalize_cand_kernel<2>
@@ -421,7 +422,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         lc.attrs = attr;
-        lc.numAttrs = overlap ? 1 : 0;
+        lc.numAttrs = (overlap && !prof) ? 1 : 0;
         if (cudaLaunchKernelEx(&lc, ffn, fp) != cudaSuccess) return CFGMS_ERR_CUDA;
     } else {
         const dim3 fgrid(c->S, a->R);
@@ -438,7 +439,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
     c->info.cta_pair = pair ? 1 : 0;
-    c->info.overlap = overlap ? 1 : 0;
+    c->info.overlap = (overlap && !prof) ? 1 : 0;
     c->info.launches_last_step = launches;
     c->info.launches_total += launches;
     c->info.h2d_bytes_last_step = 0; c->info.d2h_bytes_last_step = 0;

@@ -442,11 +442,19 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     extern __shared__ uint32_t dyn[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    // cells in the order K1 finishes them: stream-major, rows ascending (= row blocks ascending)
+    // Cells in the order K1 finishes them: stream-major; inside a stream first every EVEN row (ascending =
+    // row blocks ascending), then every odd row.  Companion rows are odd rows, so in a CFG batch the warps
+    // with nothing to do fill whole CTAs, which retire at once instead of holding resident CTAs half empty.
+    const int slots = (p.R + 1) >> 1;
+    const int per_stream = 2 * slots;
     const int cell = blockIdx.x * kCandWarps + warp;
-    const bool in_range = cell < p.R * p.S;
-    const int i = in_range ? cell / p.R : 0;
-    const int r = in_range ? cell - i * p.R : 0;
+    const bool in_grid = cell < per_stream * p.S;
+    const int i = in_grid ? cell / per_stream : 0;
+    const int rem = in_grid ? cell - i * per_stream : 0;
+    const int half = rem >= slots ? 1 : 0;
+    const int r_raw = 2 * (rem - half * slots) + half;
+    const bool in_range = in_grid && r_raw < p.R;
+    const int r = in_range ? r_raw : 0;
     const int pm = p.pair_map[r];
     const bool valid = in_range && !(pm >= 0 && (r & 1));   // a companion row is written by its cond row
 
