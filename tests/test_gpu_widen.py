@@ -1,6 +1,8 @@
 """GPU parity of the widenings against the oracle, through the C ABI:
 W1 streaming frame emission (bit-exact), W2 static logit bias + forced tokens (same tolerance
-rules as the main path), W3 feedback aggregation (correctly rounded bf16 of the exact sum)."""
+rules as the main path), W3 feedback aggregation (correctly rounded bf16 of the exact sum),
+W4 device-resident request state with automatic drain (bit-exact), W5 stream-sharded heads
+(shards merged == unsharded, bit-exact)."""
 import numpy as np
 import pytest
 import torch

@@ -1,6 +1,6 @@
 """Pins for the oracle's widening functions:
-W1 streaming frame emission, W2 static logit bias + forced tokens, W3 feedback aggregation.
-CPU only; every check compares the oracle with something other than itself."""
+W1 streaming frame emission, W2 static logit bias + forced tokens, W3 feedback aggregation,
+W4 request-state advance with automatic drain.  CPU only; every check compares the oracle with something other than itself."""
 import numpy as np
 import torch
 from scipy import stats
