@@ -1,0 +1,107 @@
+"""Seeded randomized parity sweep: random shapes and per-request sampler parameters, with and
+without vocabulary masks, forced tokens, drain and ring buffers, against the oracle through the C
+ABI.  Small sizes (the oracle computes every cell), but shapes are drawn to hit every kernel path:
+V % 32 != 0 and V % 128 != 0 (full-scan sampler, no overlap), K tails (d % 64 != 0), ragged last
+vocabulary tile, several row blocks (row_tile 64), odd row counts, greedy and unfiltered requests."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads
+from parity_util import LOGIT_TOL, DeviceWorkload
+
+pytestmark = pytest.mark.gpu
+
+
+def _case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    S = int(rng.integers(1, 11))
+    V = int(rng.choice([16, 40, 96, 128, 160, 256, 320, 384, 520, 1024]))
+    d = int(rng.choice([64, 72, 128, 200, 256, 320]))
+    pairs = int(rng.integers(0, 40))
+    singles = 2 * int(rng.integers(0 if pairs else 1, 12))
+    T = int(rng.integers(S + 2, S + 14))
+    wl = workloads.make_config(4, base_seed=seed, overrides=dict(pairs=pairs, singles=singles, d=d, S=S, V=V, T=T, mixed=True,
+                                                                 hidden_f32=False, heavy_tail=False))
+    heads = wl.head_rows()
+    # per-request sampler parameters beyond the config-4 recipe: greedy, unfiltered, k >= V, tiny and huge temperatures
+    for r in heads:
+        u = rng.random()
+        if u < 0.15:
+            wl.temp[r] = 0.0
+        elif u < 0.3:
+            wl.top_k[r] = 0
+        elif u < 0.4:
+            wl.top_k[r] = V + 3
+        elif u < 0.5:
+            wl.top_k[r] = int(rng.integers(1, V))
+        if rng.random() < 0.2:
+            wl.w[r] = float(rng.choice([0.0, 1.0, -1.5, 7.0]))
+    for r in range(wl.R):      # companions carry their cond row's parameters (ignored, reading C14)
+        if wl.pair_map[r] >= 0 and r % 2 == 1:
+            for a in (wl.w, wl.temp, wl.top_k):
+                a[r] = a[r - 1]
+    n_frames = None
+    if rng.random() < 0.6:     # drain inside the window for some requests
+        n_frames = torch.from_numpy(rng.integers(0, T, size=wl.R).astype(np.int32))
+    bias = None
+    if rng.random() < 0.5:
+        bias = rng.normal(scale=0.7, size=(S, V))
+        bias[rng.random((S, V)) < rng.choice([0.1, 0.5, 0.9])] = -np.inf
+        bias[:, int(rng.integers(0, V))] = 0.0          # at least one token stays in every stream
+        bias = bias.astype(np.float32)
+    force = None
+    if rng.random() < 0.5:
+        force = np.full((wl.R, S), -1, dtype=np.int32)
+        m = rng.random((wl.R, S)) < 0.15
+        force[m] = rng.integers(0, V + 1, size=int(m.sum()))
+    knobs = dict(row_tile=int(rng.choice([0, 0, 64])), no_candidates=bool(rng.random() < 0.25),
+                 T_cap=int(rng.choice([T, S, S + 1])))
+    return wl, n_frames, bias, force, knobs
+
+
+@pytest.mark.parametrize("seed", range(64))
+def test_random_configuration_matches_the_oracle(seed):
+    dev = torch.device("cuda:0")
+    wl, n_frames, bias, force, knobs = _case(seed)
+    dw = DeviceWorkload(wl, dev, **knobs)
+    nf_dev = None if n_frames is None else n_frames.to(dev)
+    if bias is not None:
+        dw.ctx.set_logit_bias(torch.from_numpy(bias).to(dev))
+    ft_dev = None if force is None else torch.from_numpy(force).to(dev)
+    pm = wl.pair_map.numpy()
+    n_close = n_cells = 0
+    for t in sorted({0, 1, wl.S - 1, wl.S, wl.T // 2, wl.T - 1}):
+        logits = torch.zeros((wl.R, wl.S, wl.V), dtype=torch.float32, device=dev)
+        dw.tokens.fill_(-1)
+        dw.ctx.step(dw.hidden(t), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, wl.step(t).to(dev), dw.tokens,
+                    req_id=dw.req_id, n_frames=nf_dev, delayed=dw.delayed, logits_out=logits, force_token=ft_dev)
+        dw.check_no_device_error()
+        ref = oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, wl.step(t),
+                          wl.req_id, n_frames, wl.pad_token, want_merged=True,
+                          logit_bias=None if bias is None else bias.astype(np.float64), force_token=force)
+        got, gl = dw.tokens.cpu().numpy(), logits.cpu().numpy().astype(np.float64)
+        dl = dw.delayed.cpu().numpy()
+        tau = wl.step(t).numpy()
+        for j, (c, i) in enumerate(ref.cells):
+            n_cells += 1
+            fl = int(ref.flags[j])
+            if pm[c] >= 0:
+                assert got[pm[c], i] == got[c, i]
+            assert dl[c, int(tau[c]) % dw.T_cap, i] == got[c, i]
+            if fl & oracle.FLAG_INACTIVE:
+                assert got[c, i] == wl.pad_token, (seed, t, c, i)
+            elif fl & oracle.FLAG_FORCED:
+                assert got[c, i] == force[c, i], (seed, t, c, i)
+            else:
+                m = ref.merged[j]
+                fin = np.isfinite(m)
+                assert np.array_equal(np.isneginf(gl[c, i]), np.isneginf(m))
+                assert np.max(np.abs(gl[c, i][fin] - m[fin])) <= LOGIT_TOL, (seed, t, c, i)
+                if fl & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
+                    n_close += 1
+                else:
+                    assert got[c, i] == ref.tok[j], (seed, t, c, i, got[c, i], ref.tok[j], ref.margin[j])
+    assert n_close <= 0.2 * n_cells + 5
+    dw.ctx.close()
