@@ -2,7 +2,8 @@
 without vocabulary masks, forced tokens, drain and ring buffers, against the oracle through the C
 ABI.  Small sizes (the oracle computes every cell), but shapes are drawn to hit every kernel path:
 V % 32 != 0 and V % 128 != 0 (full-scan sampler, no overlap), K tails (d % 64 != 0), ragged last
-vocabulary tile, several row blocks (row_tile 64), odd row counts, greedy and unfiltered requests."""
+vocabulary tile, several row blocks (row_tile 64), the lean GEMM with the finalize kernel as its programmatic dependent
+(force_overlap), odd row counts, greedy and unfiltered requests."""
 import numpy as np
 import pytest
 import torch
@@ -57,7 +58,7 @@ def _case(seed):
         m = rng.random((wl.R, S)) < 0.15
         force[m] = rng.integers(0, V + 1, size=int(m.sum()))
     knobs = dict(row_tile=int(rng.choice([0, 0, 64])), no_candidates=bool(rng.random() < 0.25),
-                 T_cap=int(rng.choice([T, S, S + 1])))
+                 T_cap=int(rng.choice([T, S, S + 1])), force_overlap=bool(rng.random() < 0.35))
     return wl, n_frames, bias, force, knobs
 
 
