@@ -153,6 +153,10 @@ typedef struct {
 #define CFGMS_FRAMES_UNSET 2147483647 /* n_frames value meaning "no frame count yet" (no drain)   */
 
 /*
+ * One step in flight per context: the merged-logit spill, the candidate lists and the ready counters are
+ * the context's, so calls on one context must be enqueued on one stream (or otherwise ordered); use one
+ * context per concurrent stream.  Contexts are not thread-safe; distinct contexts are independent.
+ *
  * cfgms_step — steps 1-4 above for one batch.  Every pointer in `args` is a DEVICE pointer.
  * Enqueues on `cuda_stream` (a cudaStream_t, may be NULL for the default stream); does not
  * synchronise.  Errors detected on the host: ARG, SHAPE, CUDA.  A violated pair_map contract

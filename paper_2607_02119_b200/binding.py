@@ -258,6 +258,23 @@ class Context:
         if rc != 0:
             raise CfgmsError(rc, "cfgms_set_logit_bias")
 
+    def set_stream_vocab_sizes(self, sizes, extra_bias: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """Ragged per-stream vocabularies (e.g. one SSL stream + eight codec streams of different sizes,
+        PAPER.md:104-105) on the uniform [S][V][d] layout: stream i only ever samples tokens < sizes[i].
+        Builds the -inf vocabulary mask for the padded tail (plus `extra_bias`, fp32 [S][V], if given) and
+        installs it with cfgms_set_logit_bias.  Marshalling only: the mask is applied by the library's
+        epilogue bias.  Returns the installed bias tensor (keep it alive until the call has run)."""
+        sizes = [int(x) for x in sizes]
+        if len(sizes) != self.S or any(not (1 <= x <= self.V) for x in sizes):
+            raise ValueError("sizes must hold S values in [1, V]")
+        dev = self._heads.device
+        bias = torch.zeros((self.S, self.V), dtype=torch.float32, device=dev) if extra_bias is None \
+            else extra_bias.to(device=dev, dtype=torch.float32).clone()
+        col = torch.arange(self.V, device=dev).unsqueeze(0)
+        bias.masked_fill_(col >= torch.tensor(sizes, device=dev).unsqueeze(1), float("-inf"))
+        self.set_logit_bias(bias, stream=stream)
+        return bias
+
     def feedback(self, tokens: torch.Tensor, emb: torch.Tensor, x_out: Optional[torch.Tensor] = None,
                  stream=None) -> torch.Tensor:
         """cfgms_feedback: tokens int32 [R][S], emb bf16 [S][V_e][d] -> x bf16 [R][d] (all cuda)."""

@@ -293,3 +293,31 @@ def test_stream_sharded_contexts_sample_what_the_unsharded_head_samples(dev, wor
     assert e.value.status == 1      # CFGMS_ERR_ARG
     for ctx, *_ in shards:
         ctx.close()
+
+
+# ------------------------------------------------------------------ ragged per-stream vocabularies (W2 mask)
+def test_ragged_stream_vocabularies_equal_truncated_heads(dev):
+    """OpusLM-like shape: 9 streams of different vocabulary sizes on the padded uniform layout.  With the
+    -inf tail mask installed by set_stream_vocab_sizes, every stream must sample exactly what the oracle
+    samples from that stream's TRUNCATED head (a separate oracle run per distinct size on heads[:, :V_i]),
+    i.e. padding + mask is the same computation as a ragged head."""
+    wl = _custom(pairs=4, singles=2, d=128, S=9, V=512, T=20, mixed=True)
+    wl.top_k[:] = 30
+    sizes = [512, 200, 200, 384, 64, 512, 100, 37, 256]
+    dw = DeviceWorkload(wl, dev)
+    keep = dw.ctx.set_stream_vocab_sizes(sizes)
+    for t in (9, 12):
+        dw.tokens.fill_(-1)
+        dw.step(t)
+        dw.check_no_device_error()
+        got = dw.tokens.cpu().numpy()
+        for Vi in sorted(set(sizes)):
+            ref = oracle.step(wl.heads[:, :Vi].contiguous(), wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k,
+                              wl.seed, wl.step(t), wl.req_id, wl.n_frames, wl.pad_token)
+            for j, (c, i) in enumerate(ref.cells):
+                if sizes[i] != Vi or ref.flags[j] & oracle.FLAG_INACTIVE:
+                    continue
+                assert got[c, i] < Vi
+                if not ref.flags[j] & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
+                    assert got[c, i] == ref.tok[j], (t, c, i, Vi)
+    del keep
