@@ -242,9 +242,10 @@ __device__ __forceinline__ void red_release_gpu_add(int* p, int v) {
 }
 
 // Store through a pointer whose provenance the compiler no longer sees (kept in one running
-// register): say it is global so that it does not fall back to a generic store.
+// register): say it is global so that it does not fall back to a generic store.  Streaming (.cs): the z
+// spill is written once and almost never read back, so it should not displace weight tiles in L2.
 __device__ __forceinline__ void st_global_f32(void* p, float v) {
-    asm volatile("st.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+    asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
 }
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
