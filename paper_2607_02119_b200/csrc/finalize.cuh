@@ -55,6 +55,7 @@ struct FinalizeParams {
     unsigned long long* stats;// [16] cells that arrived before their group was complete (summed on the host)
     int* err;                 // sticky error word
     int BN, num_row_blocks, ready_target;
+    int poll_ns;              // sleep between two polls of a ready counter
     int stream_base, stream_stride;   // global stream of local stream i = base + i * stride (stream-sharded heads)
 };
 
@@ -486,7 +487,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
             atomicAdd(p.stats + (blockIdx.x & 15), 1ull);   // evidence counter, spread over 16 words
             const uint64_t t0 = global_timer_ns();
             while (ld_acquire_gpu(flag) < p.ready_target) {
-                __nanosleep(200);
+                __nanosleep(p.poll_ns);
                 if (global_timer_ns() - t0 > 2000000000ull) {
                     atomicCAS(p.err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (9 << 8));
                     __threadfence_system();
