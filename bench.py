@@ -195,7 +195,7 @@ class Runner:
 
     def time_cold(self, K: int, flush):
         """Per-step device time with the L2 flushed (256 MiB written) before every step.
-        -> (graph us, eager median us).  Graph: K x (flush + step) captured in one CUDA graph minus K x flush
+        -> (graph us, (eager median, p10, p90) us).  Graph: K x (flush + step) captured in one CUDA graph minus K x flush
         captured alone, so that host launch overhead does not enter; eager: event pair around each
         eagerly launched step (includes the launch overhead of its two kernels)."""
         torch = self.torch
@@ -209,7 +209,7 @@ class Runner:
             torch.cuda.synchronize()
             times.append(e0.elapsed_time(e1) * 1e3)
         times.sort()
-        eager = times[len(times) // 2]
+        eager = (times[len(times) // 2], times[len(times) // 10], times[(9 * len(times)) // 10])   # median, p10, p90
 
         def graph_of(with_step: bool):
             g = torch.cuda.CUDAGraph()
@@ -484,7 +484,8 @@ def main():
                 cold_us, cold_eager_us = r.time_cold(48, flush)
                 t_roof = max(r.flops_per_step / (peaks["tflops"] * 1e12), r.bytes_per_step / (peaks["hbm_gbs"] * 1e9)) * 1e6
                 extras[f"config{cfg}"] = {"us_per_step_hot": hot_us, "us_per_step_cold_l2": cold_us,
-                                          "us_per_step_cold_l2_eager": cold_eager_us, "gemm_us": g_us,
+                                          "us_per_step_cold_l2_eager": cold_eager_us[0],
+                                          "us_per_step_cold_l2_eager_p10_p90": [cold_eager_us[1], cold_eager_us[2]], "gemm_us": g_us,
                                           "finalize_us": f_us, "frames_per_s_hot": r.wl.n_req / hot_us * 1e6,
                                           "roofline_us": t_roof, "frac_hot": t_roof / hot_us, "frac_cold": t_roof / cold_us}
                 if cfg in (2, 3):
