@@ -633,19 +633,31 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     for (int j = 0; j < CPL; ++j) {
                         uint32_t ovf_mask = __ballot_sync(0xffffffffu, j * 32 + lane < G && (key[j][3] | 31u) >= tE);
                         while (ovf_mask && n_list >= 0) {
-                            const int cc = j * 32 + __ffs(ovf_mask) - 1;
-                            ovf_mask &= ovf_mask - 1u;
-                            const uint32_t k32 = float_key(__ldcg(zr + cc * 32 + lane));
-                            const bool pred = k32 >= tE;
-                            const uint32_t b = __ballot_sync(0xffffffffu, pred);
-                            if (n_list + __popc(b) > cap) { n_list = -1; break; }   // too many ties: full scan
-                            if (pred) {
-                                const int pos = n_list + __popc(b & ((1u << lane) - 1u));
-                                list_key[pos] = k32;
-                                list_v[pos] = cc * 32 + lane;
+                            // up to four overflowing chunks per round: their 128-byte rows are requested together,
+                            // so a cell with several of them pays one L2 round trip, not one per chunk
+                            int cc[4];
+                            float zv[4];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                cc[u] = ovf_mask ? j * 32 + __ffs(ovf_mask) - 1 : -1;
+                                ovf_mask &= ovf_mask - 1u;        // 0 stays 0
+                                zv[u] = cc[u] >= 0 ? __ldcg(zr + cc[u] * 32 + lane) : 0.f;
                             }
-                            n_list += __popc(b);
-                            n_new += __popc(b) - 4;
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (cc[u] < 0 || n_list < 0) continue;
+                                const uint32_t k32 = float_key(zv[u]);
+                                const bool pred = k32 >= tE;
+                                const uint32_t b = __ballot_sync(0xffffffffu, pred);
+                                if (n_list + __popc(b) > cap) { n_list = -1; continue; }   // too many ties: full scan
+                                if (pred) {
+                                    const int pos = n_list + __popc(b & ((1u << lane) - 1u));
+                                    list_key[pos] = k32;
+                                    list_v[pos] = cc[u] * 32 + lane;
+                                }
+                                n_list += __popc(b);
+                                n_new += __popc(b) - 4;
+                            }
                         }
                     }
                     __syncwarp();
