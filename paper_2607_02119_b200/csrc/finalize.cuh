@@ -456,7 +456,15 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     const int r_raw = 2 * (rem - half * slots) + half;
     const bool in_range = in_grid && r_raw < p.R;
     const int r = in_range ? r_raw : 0;
+    // every per-request parameter is requested here, before any of them is used: one L2 round trip for
+    // all of them instead of one per dependent use (row r is always a readable row)
     const int pm = p.pair_map[r];
+    const int tau = p.step[r];
+    const int F_req = p.n_frames ? p.n_frames[r] : 2147483647;
+    const float temp = p.temp[r];
+    const int tk_raw = p.top_k[r];
+    const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
+    const int ft = forced_token(p, r, i);
     const bool valid = in_range && !(pm >= 0 && (r & 1));   // a companion row is written by its cond row
 
     const int V = p.V;
@@ -469,14 +477,10 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     uint32_t* list_key = reinterpret_cast<uint32_t*>(misc + 8);
     int* list_v = reinterpret_cast<int*>(list_key + cap);
 
-    const int tau = p.step[r];
     const int gi = global_stream(p, i);
-    bool active = valid && (gi <= tau) && (p.n_frames == nullptr || tau - gi < p.n_frames[r]);
+    bool active = valid && (gi <= tau) && (tau - gi < F_req);
     int token = p.pad_token;
-    if (active) {
-        const int ft = forced_token(p, r, i);
-        if (ft >= 0) { token = ft; active = false; }
-    }
+    if (active && ft >= 0) { token = ft; active = false; }
     if (valid && p.ready) {
         // Wait until K1 has written every tile of this (stream, row block): the acquire pairs with the
         // epilogue warps' red.release.  EVERY request-owning cell waits, also a PAD or forced one that
@@ -500,12 +504,9 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     if (active) {
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
         const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
-        const float temp = p.temp[r];
-        const int tk_raw = p.top_k[r];
         const bool greedy = (tk_raw == 1) || (temp == 0.f);
         const bool filter = !greedy && tk_raw > 0 && tk_raw < V;
         const int tk = greedy ? 1 : tk_raw;   // greedy = exact top-1 (ties: lowest token), no noise
-        const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
         BestSV best = {-INFINITY, 0x7fffffff};
 
         if (greedy || (filter && tk <= E)) {
