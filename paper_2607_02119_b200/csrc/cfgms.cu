@@ -374,13 +374,17 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         lc.blockDim = dim3(kGemmThreads);
         lc.dynamicSmemBytes = smem;
         lc.stream = st;
-        cudaLaunchAttribute attr[1];
+        cudaLaunchAttribute attr[2];
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = pair ? 2 : 1;
         attr[0].val.clusterDim.y = 1;
         attr[0].val.clusterDim.z = 1;
+        // the GEMM may be launched while the previous kernel of the stream still runs (it waits for it on the
+        // device before touching shared data, head_gemm.cuh): hides its launch latency and set-up
+        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[1].val.programmaticStreamSerializationAllowed = 1;
         lc.attrs = attr;
-        lc.numAttrs = 1;
+        lc.numAttrs = (c->overlap_mode == 1 || prof) ? 1 : 2;
         if (cudaLaunchKernelEx(&lc, fn, c->tmap_w, c->tmap_h, gp) != cudaSuccess) return CFGMS_ERR_CUDA;
     }
     ++launches;

@@ -242,6 +242,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
     __shared__ float red_s[kFinWarps];
     __shared__ int red_v[kFinWarps];
 
+    pdl_launch_dependents();    // the next kernel in the stream may be set up while this one runs
     const int i = blockIdx.x;   // stream
     const int r = blockIdx.y;   // batch row
     const int tid = threadIdx.x;
@@ -358,6 +359,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
     __shared__ float red_s[kFinWarps];
     __shared__ int red_v[kFinWarps];
 
+    pdl_launch_dependents();
     const int i = blockIdx.x, r = blockIdx.y, tid = threadIdx.x;
     const int pm = p.pair_map[r];
     if (pm >= 0 && (r & 1)) return;
@@ -441,6 +443,10 @@ __host__ __device__ constexpr int cand_warp_words(int V) { return 256 + 32 + 8 +
 template <int CPL>   // chunks per lane: V <= 1024 * CPL
 __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(const FinalizeParams p) {
     extern __shared__ uint32_t dyn[];
+    // The next kernel in the stream (normally the next step's head GEMM, launched as a programmatic
+    // dependent) may be scheduled and set up while this grid runs; it waits for this grid's completion
+    // (griddepcontrol.wait) before it touches anything this grid reads or writes.
+    pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     // Cells in the order K1 finishes them: stream-major; inside a stream first every EVEN row (ascending =

@@ -212,9 +212,15 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     if (kPair) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
+    // This grid may itself have been launched early, as a programmatic dependent of whatever precedes it in
+    // the stream (the previous step's finalize kernel, or the kernel that produced the hidden states): its
+    // launch latency and the set-up above then overlap that kernel's tail.  Nothing before this point reads
+    // or writes anything another kernel touches; from here on it does.
+    pdl_wait_primary();
     // Every CTA is resident from here on: let the finalize grid (K2, launched with programmatic
     // stream serialization) be scheduled beside this one.  It consumes finished (stream, row
-    // block) groups through p.ready while the GEMM is still running.
+    // block) groups through p.ready while the GEMM is still running.  (Only after the wait above: K2 of
+    // THIS step must not poll the ready counters before K2 of the previous step has re-armed them.)
     pdl_launch_dependents();
 
     if (warp == 2 && !p.split_tma) {
