@@ -214,14 +214,10 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     const uint32_t tmem_base = *tmem_ptr;
     // This grid may itself have been launched early, as a programmatic dependent of whatever precedes it in
     // the stream (the previous step's finalize kernel, or the kernel that produced the hidden states): its
-    // launch latency and the set-up above then overlap that kernel's tail.  Nothing before this point reads
-    // or writes anything another kernel touches; from here on it does.
-    pdl_wait_primary();
-    // Every CTA is resident from here on: let the finalize grid (K2, launched with programmatic
-    // stream serialization) be scheduled beside this one.  It consumes finished (stream, row
-    // block) groups through p.ready while the GEMM is still running.  (Only after the wait above: K2 of
-    // THIS step must not poll the ready counters before K2 of the previous step has re-armed them.)
-    pdl_launch_dependents();
+    // launch latency and the set-up above then overlap that kernel's tail.  Each warp role executes
+    // griddepcontrol.wait (pdl_wait_primary) right before its first access to data another kernel may
+    // produce or still read; the weight producer never needs to (the head weights are constant for the
+    // context's lifetime, include/cfgms.h), so weight tiles start streaming before the previous kernel ends.
 
     if (warp == 2 && !p.split_tma) {
         // idle: warp 0 issues both loads (see below); wait at the teardown barrier
@@ -235,6 +231,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         // weight producer of the leader posts the expected byte count of the whole stage.
         const bool load_w = warp == 0;
         const bool load_h = warp == 2 || !p.split_tma;
+        if (load_h) pdl_wait_primary();        // the hidden states may come from the preceding kernel
         const uint32_t full_sig = kPair ? mapa_shared(bar_full, 0u) : bar_full;
         const uint32_t tx_bytes = (a_bytes + b_bytes) * (kPair ? 2u : 1u);
         int s = 0;
@@ -303,6 +300,13 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         }
     } else {
         // ================= epilogue (warps 3..10, every CTA) =================
+        // batch parameters are read and z / candidates / counters written from here on
+        pdl_wait_primary();
+        // Let the finalize grid (K2, launched with programmatic stream serialization) be scheduled beside
+        // this one: it consumes finished (stream, row block) groups through p.ready while the GEMM is still
+        // running.  Only after the wait above: K2 of THIS step must not poll the ready counters before K2
+        // of the previous step has re-armed them.
+        pdl_launch_dependents();
         const int ew = warp - kCtrlWarps;
         const int quarter = warp & 3;             // TMEM lane quarter this warp may read
         const int half = ew >> 2;                 // which slab pairs (alternating) this warp takes
