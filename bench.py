@@ -28,7 +28,7 @@ METRIC = "cfg_audio_frames_per_sec"
 UNIT = "frames/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per head-GEMM launch from the committed
 # `ncu --set full` capture (profiles/), keyed by config; None until captured.
-NCU_TRAFFIC_BYTES = {5: 343.02e6}   # profiles/r1c_ncu_full_config5.md: dram read + written per head-GEMM launch
+NCU_TRAFFIC_BYTES = {5: 342.68e6}   # profiles/r1c_ncu_full_config5.md: dram read + written per head-GEMM launch
 
 
 def load_peaks():
