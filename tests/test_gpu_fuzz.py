@@ -1,4 +1,4 @@
-"""Seeded randomized parity sweep: random shapes and per-request sampler parameters, with and
+"""Seeded randomized parity sweep (160 cases): random shapes and per-request sampler parameters, with and
 without vocabulary masks, forced tokens, drain and ring buffers, against the oracle through the C
 ABI.  Small sizes (the oracle computes every cell), but shapes are drawn to hit every kernel path:
 V % 32 != 0 and V % 128 != 0 (full-scan sampler, no overlap), K tails (d % 64 != 0), ragged last
@@ -62,7 +62,7 @@ def _case(seed):
     return wl, n_frames, bias, force, knobs
 
 
-@pytest.mark.parametrize("seed", range(64))
+@pytest.mark.parametrize("seed", range(160))
 def test_random_configuration_matches_the_oracle(seed):
     dev = torch.device("cuda:0")
     wl, n_frames, bias, force, knobs = _case(seed)
