@@ -106,3 +106,27 @@ def test_random_configuration_matches_the_oracle(seed):
                     assert got[c, i] == ref.tok[j], (seed, t, c, i, got[c, i], ref.tok[j], ref.margin[j])
     assert n_close <= 0.2 * n_cells + 5
     dw.ctx.close()
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_large_configuration_sampled_cells(seed):
+    """Larger random shapes (several row blocks, CTA pairs, one to five waves of tiles — the default policy then
+    picks the serial or the overlapped launch by itself), mixed batches with per-request parameters; the oracle
+    checks a seeded sample of cells of two steps."""
+    from parity_util import ParityStats, compare_step, sample_cells
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(7000 + seed)
+    S = int(rng.choice([4, 8, 16]))
+    V = int(rng.choice([1024, 2048]))
+    d = int(rng.choice([512, 1024]))
+    pairs = int(rng.integers(60, 300))
+    singles = 2 * int(rng.integers(0, 60))
+    wl = workloads.make_config(4, base_seed=100 + seed, overrides=dict(pairs=pairs, singles=singles, d=d, S=S, V=V, T=64,
+                                                                       mixed=True, hidden_f32=False, heavy_tail=bool(seed & 1)))
+    dw = DeviceWorkload(wl, dev)
+    stats = ParityStats()
+    for n, t in enumerate((S - 1, 33)):
+        compare_step(dw, t, sample_cells(wl, 96, seed=seed * 10 + n), stats)
+    print(f"large fuzz {seed}: R={wl.R} S={S} V={V} d={d} {dw.ctx.info()['row_blocks']} row blocks, overlap={dw.ctx.info()['overlap']}:",
+          stats.summary())
+    dw.ctx.close()
