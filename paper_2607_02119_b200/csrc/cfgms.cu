@@ -72,6 +72,10 @@ struct cfgms_ctx {
     cudaEvent_t* prof_ev = nullptr;   // [kProfMax][3]
     int prof_n = 0;
     cfgms_info info;
+#ifdef CFGMS_TRACE
+    unsigned long long* trace_k1 = nullptr;
+    unsigned long long* trace_k2 = nullptr;
+#endif
 };
 
 namespace {
@@ -289,7 +293,8 @@ void cfgms_destroy(cfgms_ctx* c) {
     cudaFree(c->err);
     cudaFree(c->ready);
     if (c->prof_ev) {
-        for (int j = 0; j < 3 * kProfMax; ++j) cudaEventDestroy(c->prof_ev[j]);
+        for (int j = 0; j < 3 * kProfMax; ++j)
+            if (c->prof_ev[j]) cudaEventDestroy(c->prof_ev[j]);
         delete[] c->prof_ev;
     }
     HostStage& h = c->hs;
@@ -356,6 +361,9 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;
     const int grid = pair ? 2 * workers : workers;
+#ifdef CFGMS_TRACE
+    gp.trace = c->trace_k1;
+#endif
     const size_t smem = GemmSmemLayout::total(b_rows, stages);
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
     {
@@ -409,6 +417,9 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.BN = BN; fp.num_row_blocks = nrb;
     fp.stream_base = c->stream_base; fp.stream_stride = c->stream_stride;
     fp.poll_ns = c->poll_ns;
+#ifdef CFGMS_TRACE
+    fp.trace = c->trace_k2;
+#endif
     fp.ready_target = (c->V / kBM) * kEpiWarps;   // every epilogue warp of every vocabulary tile of the stream
     if (c->use_cand) {
         const size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;
@@ -591,10 +602,16 @@ int cfgms_last_device_error(cfgms_ctx* c, int32_t* row_out) {
 int cfgms_profile_enable(cfgms_ctx* c, int on) {
     if (!c) return CFGMS_ERR_ARG;
     if (on && !c->prof_ev) {
-        c->prof_ev = new (std::nothrow) cudaEvent_t[3 * kProfMax];
-        if (!c->prof_ev) return CFGMS_ERR_NOMEM;
-        for (int j = 0; j < 3 * kProfMax; ++j)
-            if (cudaEventCreate(&c->prof_ev[j]) != cudaSuccess) return CFGMS_ERR_CUDA;
+        cudaEvent_t* ev = new (std::nothrow) cudaEvent_t[3 * kProfMax]();    // value-initialised: null handles
+        if (!ev) return CFGMS_ERR_NOMEM;
+        for (int j = 0; j < 3 * kProfMax; ++j) {
+            if (cudaEventCreate(&ev[j]) != cudaSuccess) {
+                for (int q = 0; q < j; ++q) cudaEventDestroy(ev[q]);
+                delete[] ev;
+                return CFGMS_ERR_CUDA;
+            }
+        }
+        c->prof_ev = ev;
     }
     c->prof_on = on != 0;
     c->prof_n = 0;
@@ -629,6 +646,15 @@ int cfgms_overlap_stats(cfgms_ctx* c, int64_t* cells_waited) {
     for (int j = 0; j < 16; ++j) *cells_waited += static_cast<int64_t>(w[j]);
     return CFGMS_OK;
 }
+
+#ifdef CFGMS_TRACE
+// developer build only: device buffers of 16 x u64 per CTA that K1 / K2 fill with their timeline marks
+int cfgms_debug_trace(cfgms_ctx* c, unsigned long long* k1, unsigned long long* k2) {
+    if (!c) return CFGMS_ERR_ARG;
+    c->trace_k1 = k1; c->trace_k2 = k2;
+    return CFGMS_OK;
+}
+#endif
 
 int cfgms_get_info(cfgms_ctx* c, cfgms_info* out) {
     if (!c || !out) return CFGMS_ERR_ARG;

@@ -1,18 +1,25 @@
 // K2 — top-k threshold, Gumbel-max over Philox4x32-10 noise, companion token sync and the
 // delay-layout write (rows a3-a4 of DESIGN.md's hot-path table).
 //
-// One CTA of 256 threads per (request-owning batch row, stream).  The row's V temperature-
-// scaled merged logits z (fp32, written by K1, normally still L2-resident) are loaded ONCE
-// into registers as order-preserving 32-bit keys.  Exact top-k threshold without sorting V
-// values and without hammering shared-memory atomics:
-//   1. every thread takes the max of its V/256 keys; every warp extracts the ceil(k/8)-th
-//      largest of its 32 thread maxima (redux.sync loop).  The minimum L of the 8 warp values
-//      is a LOWER BOUND of the k-th largest key (at least 8*ceil(k/8) >= k keys are >= L);
-//   2. keys >= L are compacted to shared memory (about 2k candidates in practice);
-//   3. one warp runs an exact MSB-first 8-bit radix select on the candidates only;
-//   4. survivors (key >= threshold; ties kept) draw Gumbel noise; block argmax, lowest index
-//      on ties.
-// k > 256 (or V tiny) degrades gracefully: L = 0 and every key is a candidate.
+// Two samplers with identical semantics (readings C8-C12):
+//
+//  * cfgms_finalize_cand_kernel (the hot path: V % 32 == 0, V <= 8192) — ONE WARP per
+//    (request-owning row, stream) cell, working on the V/8 values K1's epilogue emitted (top-4 of every
+//    32-token chunk) instead of all V logits; chunks that may hide a top-k member are re-read from the
+//    z spill.  Described in full above the kernel, further down in this file.
+//
+//  * cfgms_finalize_kernel<EPT> / cfgms_finalize_large_kernel (every other shape, and
+//    CFGMS_CFG_NO_CANDIDATES) — one CTA of 256 threads per cell.  The row's V temperature-scaled
+//    merged logits z (fp32, written by K1, normally still L2-resident) are loaded ONCE into registers
+//    as order-preserving 32-bit keys.  Exact top-k threshold without sorting V values:
+//      1. every thread takes the max of its V/256 keys; every warp extracts the ceil(k/8)-th
+//         largest of its 32 thread maxima (redux.sync loop).  The minimum L of the 8 warp values
+//         is a LOWER BOUND of the k-th largest key (at least 8*ceil(k/8) >= k keys are >= L);
+//      2. keys >= L are compacted to shared memory (about 2k candidates in practice);
+//      3. one warp runs an exact MSB-first 8-bit radix select on the candidates only;
+//      4. survivors (key >= threshold; ties kept) draw Gumbel noise; block argmax, lowest index
+//         on ties.
+//    k > 256 (or V tiny) degrades gracefully: L = 0 and every key is a candidate.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -57,6 +64,9 @@ struct FinalizeParams {
     int BN, num_row_blocks, ready_target;
     int poll_ns;              // sleep between two polls of a ready counter
     int stream_base, stream_stride;   // global stream of local stream i = base + i * stride (stream-sharded heads)
+#ifdef CFGMS_TRACE
+    unsigned long long* trace;
+#endif
 };
 
 // Philox4x32-10 (Salmon et al. 2011): ten rounds of two 32x32->64 multiplies with key bumps.
@@ -449,6 +459,13 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     pdl_launch_dependents();
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+#ifdef CFGMS_TRACE
+    const bool tr = threadIdx.x == 0;
+    if (tr) { CFGMS_TRACE_MARK(p.trace, 0); CFGMS_TRACE_MARK(p.trace, 1); }
+#define CFGMS_K2_MARK(slot) do { if (tr) CFGMS_TRACE_MARK(p.trace, slot); } while (0)
+#else
+#define CFGMS_K2_MARK(slot) ((void)0)
+#endif
     // Cells in the order K1 finishes them: stream-major; inside a stream first every EVEN row (ascending =
     // row blocks ascending), then every odd row.  Companion rows are odd rows, so in a CFG batch the warps
     // with nothing to do fill whole CTAs, which retire at once instead of holding resident CTAs half empty.
@@ -507,6 +524,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         }
         __syncwarp();
     }
+    CFGMS_K2_MARK(2);      // parameters in, readiness wait over
     if (active) {
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
         const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
@@ -531,6 +549,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     key[j][0] = key[j][1] = key[j][2] = key[j][3] = 0u;
                 }
             }
+            CFGMS_K2_MARK(3);      // emitted values loaded
             {
                 // ---- t_E: k-th largest of the E emitted values
                 const int jj = (tk + G - 1) / G - 1;           // 0..3: the (jj+1)-th value of every chunk
@@ -613,6 +632,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     tE = E <= cap ? warp_radix_select(SmemKeys{list_key}, E, tk, hist, lane) : 0u;
                     __syncwarp();
                 }
+                CFGMS_K2_MARK(4);  // t_E known
                 // ---- candidate list {z >= t_E}; overflowing chunks are re-read in full
                 int n_list = 0;
                 uint32_t any_overflow = 0u;
@@ -634,8 +654,8 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     }
                 }
                 uint32_t thr = tE;
+                CFGMS_K2_MARK(5);  // list built
                 if (any_overflow) {
-                    int n_new = 0;   // values >= t_E that were hidden behind a chunk's four emitted ones
 #pragma unroll
                     for (int j = 0; j < CPL; ++j) {
                         uint32_t ovf_mask = __ballot_sync(0xffffffffu, j * 32 + lane < G && (key[j][3] | 31u) >= tE);
@@ -663,13 +683,16 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                                     list_v[pos] = cc[u] * 32 + lane;
                                 }
                                 n_list += __popc(b);
-                                n_new += __popc(b) - 4;
                             }
                         }
                     }
                     __syncwarp();
-                    if (n_list >= 0 && n_new > 0) {
-                        // exact threshold of the completed set = its k-th largest: drop the (n_list - k) smallest
+                    if (n_list > tk) {
+                        // More than k values >= t_E: a re-read chunk revealed values its four emitted ones had
+                        // hidden (or several values tie at t_E).  The completed set holds every z >= t_E, so the
+                        // exact threshold is its k-th largest: drop the (n_list - k) smallest.  (Deciding this by
+                        // the list length, not by per-chunk bookkeeping, stays exact when a chunk's 4th emitted
+                        // value shares t_E's 27-bit bucket but lies below t_E.)
                         const int extra = n_list - tk;
                         if (extra <= 8) {
                             for (int it = 0;; ++it) {
@@ -695,6 +718,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     }
                 }
                 __syncwarp();
+                CFGMS_K2_MARK(6);  // overflow chunks handled, exact threshold known
                 if (n_list >= 0) {
                     for (int e = lane; e < n_list; e += 32) {
                         const uint32_t ck = list_key[e];
@@ -724,8 +748,10 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         }
         best = warp_argmax(best);
         token = best.v;
+        CFGMS_K2_MARK(7);          // noise drawn, argmax done
     }
     if (valid && lane == 0) write_cell(p, r, i, pm, tau, token);
+    CFGMS_K2_MARK(8);
     if (p.ready) {
         // the last CTA to finish re-arms the counters for the next step's K1 (which starts after this grid)
         __syncthreads();

@@ -77,6 +77,9 @@ struct GemmParams {
     int V;               // tokens per stream (ready != nullptr requires V % kBM == 0)
     int split_tma;       // 1: warp 2 issues the row-tile loads; 0: warp 0 issues both (warp 2 idles)
     uint64_t policy_w, policy_h;
+#ifdef CFGMS_TRACE
+    unsigned long long* trace;
+#endif
 };
 
 struct GemmSmemLayout {
@@ -191,6 +194,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     const int worker = kPair ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
     const int num_workers = kPair ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
 
+    if (threadIdx.x == 0) { CFGMS_TRACE_MARK(p.trace, 0); CFGMS_TRACE_MARK(p.trace, 1); }
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmap_w);
         tma_prefetch_desc(&tmap_h);
@@ -212,6 +216,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     if (kPair) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
+    if (threadIdx.x == 0) CFGMS_TRACE_MARK(p.trace, 2);          // set-up done
     // This grid may itself have been launched early, as a programmatic dependent of whatever precedes it in
     // the stream (the previous step's finalize kernel, or the kernel that produced the hidden states): its
     // launch latency and the set-up above then overlap that kernel's tail.  Each warp role executes
@@ -232,6 +237,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         const bool load_w = warp == 0;
         const bool load_h = warp == 2 || !p.split_tma;
         if (load_h) pdl_wait_primary();        // the hidden states may come from the preceding kernel
+        if (load_h && lane == 0) CFGMS_TRACE_MARK(p.trace, 3);   // previous kernel done (row producer)
         const uint32_t full_sig = kPair ? mapa_shared(bar_full, 0u) : bar_full;
         const uint32_t tx_bytes = (a_bytes + b_bytes) * (kPair ? 2u : 1u);
         int s = 0;
@@ -277,6 +283,9 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 for (int kb = 0; kb < p.num_kb; ++kb) {
                     mbar_wait(bar_full + 8 * s, phase, p.err, 3);
                     tc_fence_after();
+                    if (lane == 0 && tile == worker && kb == 0) CFGMS_TRACE_MARK(p.trace, 4);            // first stage landed
+                    if (lane == 0 && tile == worker && kb == p.num_kb / 2) CFGMS_TRACE_MARK(p.trace, 5); // half of the first tile
+                    if (lane == 0 && tile == worker && kb == p.num_kb - 1) CFGMS_TRACE_MARK(p.trace, 6); // last stage of the first tile landed
                     if (elect_one()) {
                         // the start-address field counts 16-byte units
                         const uint64_t a_desc = a_desc0 + static_cast<uint64_t>((s * a_bytes) >> 4);
@@ -352,6 +361,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
 
             mbar_wait(bar_tfull + 8 * acc, acc_phase, p.err, 4);
             tc_fence_after();
+            if (warp == kCtrlWarps && lane == 0 && tile == worker) CFGMS_TRACE_MARK(p.trace, 7);      // first accumulator complete
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * BN;
             if (half >= nsp) {                            // nothing to read for this warp: release at once
                 tc_fence_before();
@@ -449,8 +459,10 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 __syncwarp();
                 if (lane == 0) red_release_gpu_add(p.ready + ((vt * kBM) / p.V) * p.num_row_blocks + rb, 1);
             }
+            if (warp == kCtrlWarps && lane == 0 && tile == worker) CFGMS_TRACE_MARK(p.trace, 8);      // first epilogue done
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
+        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 9);                            // all epilogues done
     }
 
     tc_fence_before();
@@ -459,6 +471,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         tc_fence_after();
         if (kPair) tmem_dealloc_pair(tmem_base, kTmemCols); else tmem_dealloc(tmem_base, kTmemCols);
     }
+    if (threadIdx.x == 0) CFGMS_TRACE_MARK(p.trace, 10);
 }
 
 // Full register budget (168): the fastest GEMM, but nothing else fits on its SMs while it runs.

@@ -253,6 +253,17 @@ __device__ __forceinline__ void st_global_f32(void* p, float v) {
     asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
 }
 
+// Developer timeline (compiled in only with -DCFGMS_TRACE; the product build contains none of it):
+// slot 0 of a CTA's 16-word record holds %globaltimer at entry, slots 1.. hold %clock64 at the marks.
+#ifdef CFGMS_TRACE
+__device__ __forceinline__ void trace_mark(unsigned long long* trace, int slot) {
+    if (trace) trace[blockIdx.x * 16 + slot] = slot == 0 ? global_timer_ns() : static_cast<unsigned long long>(clock64());
+}
+#define CFGMS_TRACE_MARK(trace, slot) trace_mark(trace, slot)
+#else
+#define CFGMS_TRACE_MARK(trace, slot) ((void)0)
+#endif
+
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }

@@ -69,6 +69,36 @@ def sample_cells(wl, n_cells, seed):
     return allc[idx]
 
 
+CLOSE_FRAC_MAX = 0.03   # SURVEY 8(c) acceptance 2 expects 0.5-1.2 % close ties at the BASELINE shapes
+
+
+def valid_alternative(wl, t, c, i, tok_gpu, logit_bias=None, tol=oracle.TOL):
+    """For a cell the oracle flags close / boundary the GPU may pick another token — but only a
+    token that a perturbation of z by < tol could have made win: it must lie inside the top-k
+    set up to tol, `z[tok] >= thr - tol`, and its perturbed score must reach the oracle's best
+    up to twice tol (both competitors may move), `z[tok] + g(tok) >= s_best - 2 tol`.  Greedy
+    cells: `M[tok] >= max M - 2 tol`.  Recomputed from the oracle's own pieces for this one cell."""
+    if not (0 <= tok_gpu < wl.V):
+        return False
+    hid = oracle.f32_to_bf16(wl.hidden(t)) if wl.hidden_f32 else wl.hidden(t)
+    u = int(wl.pair_map[c])
+    M = oracle.logits_row(wl.heads, wl.embeds, hid, int(c), int(i))
+    if u >= 0:
+        M = oracle.cfg_merge(M, oracle.logits_row(wl.heads, wl.embeds, hid, u, int(i)), float(wl.w[c]))
+    if logit_bias is not None:
+        M = M + np.asarray(logit_bias, dtype=np.float64)[i]
+    temp, tk = float(wl.temp[c]), int(wl.top_k[c])
+    tau = int(wl.step(t)[c])
+    rid = int(wl.req_id[c]) & 0xFFFFFFFF
+    tok, _, flags, thr = oracle.sample_cell(M, temp, tk, wl.seed, rid, tau, int(i), tol)
+    if flags & oracle.FLAG_GREEDY:
+        return bool(M[tok_gpu] >= M[tok] - 2 * tol)
+    z = M / float(np.float32(temp))
+    g = lambda v: oracle.gumbel(wl.seed, rid, tau, int(i), int(v))
+    s_best = z[tok] + g(tok)
+    return bool(z[tok_gpu] >= thr - tol and z[tok_gpu] + g(tok_gpu) >= s_best - 2 * tol)
+
+
 class ParityStats:
     def __init__(self):
         self.n = self.n_pad = self.n_close = self.n_close_mismatch = self.n_tight_mismatch = 0
@@ -76,6 +106,14 @@ class ParityStats:
         self.sq_err = 0.0
         self.n_logits = 0
         self.first_mismatch = None
+
+    def assert_close_fraction(self, frac=CLOSE_FRAC_MAX, slack=2):
+        """Close ties are counted and reported, not failed — but they must stay the rare event the
+        margin statistics predict, and a differing close cell was already checked to hold a valid
+        alternative (compare_step)."""
+        n_sampled = self.n - self.n_pad
+        assert self.n_close_mismatch <= self.n_close
+        assert self.n_close <= frac * n_sampled + slack, f"{self.n_close} close ties among {n_sampled} sampled cells"
 
     def summary(self):
         rmse = (self.sq_err / max(self.n_logits, 1)) ** 0.5
@@ -123,6 +161,9 @@ def compare_step(dw: DeviceWorkload, t: int, cells, stats: ParityStats, check_lo
                 stats.n_close_mismatch += 1
                 if stats.first_mismatch is None:
                     stats.first_mismatch = (t, int(c), int(i))
+                assert valid_alternative(wl, t, c, i, int(got[c, i])), (
+                    f"close cell at step {t} row {c} stream {i}: gpu token {got[c, i]} is not a valid alternative "
+                    f"to the oracle's {ref.tok[j]} (margin {ref.margin[j]})")
         else:
             assert got[c, i] == ref.tok[j], (f"token mismatch at step {t} row {c} stream {i}: gpu {got[c, i]} "
                                              f"oracle {ref.tok[j]} margin {ref.margin[j]}")

@@ -10,7 +10,7 @@ import torch
 
 import oracle
 import workloads
-from parity_util import LOGIT_TOL, DeviceWorkload
+from parity_util import LOGIT_TOL, DeviceWorkload, valid_alternative
 
 pytestmark = pytest.mark.gpu
 
@@ -72,7 +72,7 @@ def test_random_configuration_matches_the_oracle(seed):
         dw.ctx.set_logit_bias(torch.from_numpy(bias).to(dev))
     ft_dev = None if force is None else torch.from_numpy(force).to(dev)
     pm = wl.pair_map.numpy()
-    n_close = n_cells = 0
+    n_close = n_cells = n_close_mismatch = 0
     for t in sorted({0, 1, wl.S - 1, wl.S, wl.T // 2, wl.T - 1}):
         logits = torch.zeros((wl.R, wl.S, wl.V), dtype=torch.float32, device=dev)
         dw.tokens.fill_(-1)
@@ -102,9 +102,14 @@ def test_random_configuration_matches_the_oracle(seed):
                 assert np.max(np.abs(gl[c, i][fin] - m[fin])) <= LOGIT_TOL, (seed, t, c, i)
                 if fl & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
                     n_close += 1
+                    if got[c, i] != ref.tok[j]:      # a differing close cell must still hold a token that could have won
+                        n_close_mismatch += 1
+                        assert valid_alternative(wl, t, c, i, int(got[c, i]), logit_bias=bias), (seed, t, c, i, got[c, i], ref.tok[j])
                 else:
                     assert got[c, i] == ref.tok[j], (seed, t, c, i, got[c, i], ref.tok[j], ref.margin[j])
-    assert n_close <= 0.2 * n_cells + 5
+    # tiny vocabularies with masks leave few survivors per cell, so close ties are far more frequent here than at the
+    # BASELINE shapes (bounded at 3 % there, tests/test_gpu_parity.py)
+    assert n_close_mismatch <= n_close <= 0.2 * n_cells + 5
     dw.ctx.close()
 
 
@@ -129,4 +134,5 @@ def test_random_large_configuration_sampled_cells(seed):
         compare_step(dw, t, sample_cells(wl, 96, seed=seed * 10 + n), stats)
     print(f"large fuzz {seed}: R={wl.R} S={S} V={V} d={d} {dw.ctx.info()['row_blocks']} row blocks, overlap={dw.ctx.info()['overlap']}:",
           stats.summary())
+    stats.assert_close_fraction(frac=0.08)      # per-request top_k in {1, 20, 50} and temp down to 0.6: more edge cases than config 5
     dw.ctx.close()

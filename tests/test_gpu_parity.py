@@ -7,7 +7,7 @@ import torch
 
 import oracle
 import workloads
-from parity_util import DeviceWorkload, ParityStats, compare_step, sample_cells
+from parity_util import CLOSE_FRAC_MAX, DeviceWorkload, ParityStats, compare_step, sample_cells, valid_alternative
 
 pytestmark = pytest.mark.gpu
 
@@ -48,41 +48,72 @@ def test_config2_mid_and_cfg_off_twin(dev):
     for t in workloads.parity_steps(2, wl.T, wl.S):
         compare_step(dw, t, None, stats)
     print("config2:", stats.summary())
-    assert stats.n_close < 0.06 * stats.n
+    stats.assert_close_fraction()
     off = workloads.cfg_off_twin(wl)
     dwo = DeviceWorkload(off, dev)
     so = ParityStats()
     for t in (0, 9, 130):
         compare_step(dwo, t, None, so)
     print("config2 cfg-off:", so.summary())
+    # Without the w = 3 extrapolation the merged logits are ~3.6x narrower (std 1 instead of sqrt(9 + 4)), so the
+    # top-50 perturbed scores lie ~3.6x denser and ties within 2e-2 are that much more frequent (observed 5.6 %).
+    so.assert_close_fraction(frac=0.08)
+
+
+def _full_step(cfg, T, S):
+    """The parity step on which EVERY (request, stream) cell is checked (logits and tokens): the seeded
+    mid-run step, where all streams are active.  The other parity steps check a seeded sample of cells."""
+    steps = workloads.parity_steps(cfg, T, S)
+    mid = [t for t in steps if S < t < T - S]
+    return mid[0] if mid else steps[len(steps) // 2]
 
 
 def test_config3_7b_head_heavy_tail(dev):
     wl = workloads.make_config(3)
     dw = DeviceWorkload(wl, dev)
     stats = ParityStats()
+    full = _full_step(3, wl.T, wl.S)
     for n, t in enumerate(workloads.parity_steps(3, wl.T, wl.S)):
-        compare_step(dw, t, sample_cells(wl, 160, seed=30 + n), stats)
+        compare_step(dw, t, None if t == full else sample_cells(wl, 160, seed=30 + n), stats)   # full: all 1024 cells
     print("config3:", stats.summary())
+    assert stats.n >= wl.n_req * wl.S
+    stats.assert_close_fraction()
 
 
 def test_config4_mixed_continuous_batch(dev):
     wl = workloads.make_config(4)
     dw = DeviceWorkload(wl, dev)
-    stats = ParityStats()
+    # Two populations, counted apart: sampled cells of CFG pairs (the population SURVEY 8(c) simulated: 0.5-1.2 %
+    # of them within 2e-2), and cells of unpaired or greedy requests, whose un-extrapolated logits are 2-5x
+    # narrower (ties within 2e-2 that much denser; a greedy cell is close whenever the top-2 gap of M is: ~8 %
+    # at V = 2048).
+    pm, tk = wl.pair_map.numpy(), wl.top_k.numpy()
+    is_cfg = lambda cells: np.asarray([pm[c] >= 0 and tk[c] != 1 for c, _ in cells])
+    cfg_stats, rest_stats = ParityStats(), ParityStats()
+    full = _full_step(4, wl.T, wl.S)
     for n, t in enumerate(workloads.parity_steps(4, wl.T, wl.S)):
-        compare_step(dw, t, sample_cells(wl, 320, seed=40 + n), stats)
-    print("config4:", stats.summary())
-    assert stats.n_pad > 0          # step 0 has not-yet-started streams for low-offset rows
+        cells = sample_cells(wl, None if t == full else 320, seed=40 + n)      # full: all 2048 cells
+        m = is_cfg(cells)
+        compare_step(dw, t, cells[m], cfg_stats)
+        compare_step(dw, t, cells[~m], rest_stats)
+    print("config4 cfg pairs:", cfg_stats.summary())
+    print("config4 unpaired / greedy:", rest_stats.summary())
+    assert cfg_stats.n_pad + rest_stats.n_pad > 0          # step 0 has not-yet-started streams for low-offset rows
+    assert cfg_stats.n + rest_stats.n >= wl.n_req * wl.S
+    cfg_stats.assert_close_fraction()
+    rest_stats.assert_close_fraction(frac=0.10)
 
 
 def test_config5_large_batch(dev):
     wl = workloads.make_config(5)
     dw = DeviceWorkload(wl, dev)
     stats = ParityStats()
+    full = _full_step(5, wl.T, wl.S)
     for n, t in enumerate(workloads.parity_steps(5, wl.T, wl.S)):
-        compare_step(dw, t, sample_cells(wl, 160, seed=50 + n), stats)
+        compare_step(dw, t, None if t == full else sample_cells(wl, 160, seed=50 + n), stats)   # full: all 8192 cells
     print("config5:", stats.summary())
+    assert stats.n >= wl.n_req * wl.S
+    stats.assert_close_fraction()
     info = dw.ctx.info()
     assert info["row_blocks"] == 4 and info["row_tile"] == 256
 
@@ -390,7 +421,7 @@ def test_bench_launch_configuration_graph_replay(dev, cfg, n_cells):
     dw.check_no_device_error()
     assert dw.ctx.info()["overlap"] == (1 if cfg == 5 else 0)
     delayed = dw.delayed.cpu().numpy()
-    n_close = n_mismatch = 0
+    n_close = n_mismatch = n_sampled = 0
     for n, t in enumerate(steps):
         cells = sample_cells(wl, n_cells, seed=900 + n)
         ref = oracle.step(wl.heads, wl.embeds, wl.hidden(t), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, wl.step(t),
@@ -398,9 +429,16 @@ def test_bench_launch_configuration_graph_replay(dev, cfg, n_cells):
         tau = wl.step(t).numpy()
         for j, (c, i) in enumerate(ref.cells):
             got = delayed[c, int(tau[c]) % dw.T_cap, i]
+            if ref.flags[j] & oracle.FLAG_INACTIVE:
+                assert got == wl.pad_token
+                continue
+            n_sampled += 1
             if ref.flags[j] & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
                 n_close += 1
-                n_mismatch += int(got != ref.tok[j])
+                if got != ref.tok[j]:
+                    n_mismatch += 1
+                    assert valid_alternative(wl, t, c, i, int(got)), (t, c, i, got, ref.tok[j], ref.margin[j])
             else:
                 assert got == ref.tok[j], (t, c, i, got, ref.tok[j], ref.margin[j])
-    print(f"config{cfg} graph replay: close ties {n_close}, of which differ {n_mismatch}")
+    print(f"config{cfg} graph replay: {n_sampled} sampled cells, close ties {n_close}, of which differ {n_mismatch}")
+    assert n_mismatch <= n_close <= CLOSE_FRAC_MAX * n_sampled + 2

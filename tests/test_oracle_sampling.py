@@ -218,3 +218,25 @@ def test_close_and_boundary_flags():
         assert bool(flags & oracle.FLAG_BOUNDARY) == expect
         hits += int(expect)
     assert 0 < hits < 200
+
+
+def test_gumbel_key_layout_reading_c12():
+    """Reading C12 pins WHICH Philox block and word serve a token: counter = (v >> 2, tau, stream, req_id),
+    key = (seed low word, seed high word), output word v & 3.  The keyed entry point must equal the
+    composition of the separately pinned pieces (Philox vs the toolkit's generator, the uniform map,
+    the Gumbel closed forms) — a swapped counter word or key half would pass every other pin."""
+    rng = np.random.default_rng(21)
+    gfu = oracle.lib().oracle_gumbel_from_uniform
+    for _ in range(400):
+        seed = int(rng.integers(0, 2 ** 63)) * 2 + int(rng.integers(0, 2))
+        req = int(rng.integers(0, 2 ** 32))
+        tau = int(rng.integers(0, 2 ** 20))
+        stream = int(rng.integers(0, 64))
+        v = int(rng.integers(0, 2 ** 16))
+        block = oracle.philox4x32_10([v >> 2, tau, stream, req], [seed & 0xFFFFFFFF, seed >> 32])
+        want = gfu(oracle.uniform(int(block[v & 3])))
+        assert oracle.gumbel(seed, req, tau, stream, v) == want
+    # the five key parts are not interchangeable: swapping any two that differ changes the draw
+    base = oracle.gumbel(5, 1, 2, 3, 16)
+    assert len({base, oracle.gumbel(5, 2, 1, 3, 16), oracle.gumbel(5, 1, 3, 2, 16), oracle.gumbel(5, 3, 2, 1, 16),
+                oracle.gumbel(5, 1, 2, 4, 12), oracle.gumbel(1, 5, 2, 3, 16), oracle.gumbel(5 << 32, 1, 2, 3, 16)}) == 7
