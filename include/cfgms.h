@@ -64,6 +64,12 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
                                     (candidate path with V % 128 == 0)                                 */
 #define CFGMS_CFG_OVERLAP 32u    /* tuning/debug: overlap whenever eligible, even for a one-wave GEMM   */
 
+#define CFGMS_CFG_NO_PDL_FINALIZE 64u /* tuning/debug: always launch the finalize kernel as an ordinary stream-ordered
+                                    kernel.  Default for small finalize grids that do not overlap the GEMM
+                                    through the ready counters: programmatic dependent launch — scheduled while
+                                    the GEMM runs, it fetches its per-request parameters and waits on the device
+                                    (griddepcontrol.wait) for the GEMM's results                          */
+
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
     int32_t pad_token; /* written at inactive (step, stream) cells when CFGMS_CFG_PAD_TOKEN      */

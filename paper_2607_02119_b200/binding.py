@@ -19,6 +19,7 @@ CFGMS_CFG_SINGLE_CTA = 4
 CFGMS_CFG_CTA_PAIR = 8
 CFGMS_CFG_NO_OVERLAP = 16
 CFGMS_CFG_OVERLAP = 32
+CFGMS_CFG_NO_PDL_FINALIZE = 64
 CFGMS_FRAMES_UNSET = 2 ** 31 - 1
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
@@ -144,7 +145,8 @@ class Context:
     def __init__(self, heads: torch.Tensor, embeds: torch.Tensor, max_rows: int = 1024,
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
                  cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0,
-                 force_overlap: bool = False, stream_base: int = 0, stream_stride: int = 0):
+                 force_overlap: bool = False, stream_base: int = 0, stream_stride: int = 0,
+                 no_pdl_finalize: bool = False):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -167,6 +169,8 @@ class Context:
             cfg.flags |= CFGMS_CFG_NO_OVERLAP
         elif force_overlap:        # tuning: overlap even for a one-wave GEMM
             cfg.flags |= CFGMS_CFG_OVERLAP
+        if no_pdl_finalize:        # tuning: finalize kernel always as an ordinary stream-ordered launch
+            cfg.flags |= CFGMS_CFG_NO_PDL_FINALIZE
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):

@@ -47,6 +47,7 @@ struct cfgms_ctx {
     int stream_base = 0, stream_stride = 1;   // stream-sharded heads: global stream of local stream i
     int poll_ns = 2000;       // K2's sleep between polls of a ready counter: 1-4 us measured ~2.4 % faster than 50-200 ns at config 5
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
+    bool pdl_finalize = true;         // serial mode: launch a small K2 grid as a programmatic dependent of K1
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT] what the epilogue adds: bias_base (+ the caller's logit bias)
     float* bias_base = nullptr;       // [NT] W_i e_i, folded at create
@@ -219,6 +220,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     }
     cudaMemset(c->err, 0, 2 * sizeof(int));
     c->overlap_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_OVERLAP)) ? 2 : 0;
+    c->pdl_finalize = !(cfg && (cfg->flags & CFGMS_CFG_NO_PDL_FINALIZE));
     c->overlap = c->use_cand && (V % kBM) == 0 && c->overlap_mode != 1;
     if (c->overlap) {
         c->ready_words = ((S * ((c->max_rows + 63) / 64) + 1 + 1) & ~1) + 32;   // counters | done | pad | stats (16 x u64)
@@ -262,8 +264,11 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<true, false>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<false, true>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<true, true>));
-    if (!attr_ok ||
-        cudaFuncSetAttribute(cfgms_finalize_cand_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess) {
+    set_smem(reinterpret_cast<const void*>(cfgms_finalize_cand_kernel<1>));
+    set_smem(reinterpret_cast<const void*>(cfgms_finalize_cand_kernel<2>));
+    set_smem(reinterpret_cast<const void*>(cfgms_finalize_cand_kernel<4>));
+    set_smem(reinterpret_cast<const void*>(cfgms_finalize_cand_kernel<8>));
+    if (!attr_ok) {
         cfgms_destroy(c);
         return CFGMS_ERR_CUDA;
     }
@@ -417,14 +422,29 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.BN = BN; fp.num_row_blocks = nrb;
     fp.stream_base = c->stream_base; fp.stream_stride = c->stream_stride;
     fp.poll_ns = c->poll_ns;
+    fp.pdl_wait = 0;
 #ifdef CFGMS_TRACE
     fp.trace = c->trace_k2;
 #endif
     fp.ready_target = (c->V / kBM) * kEpiWarps;   // every epilogue warp of every vocabulary tile of the stream
     if (c->use_cand) {
-        const size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;
+        size_t fsmem = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4;
         const int cells = 2 * ((a->R + 1) / 2) * c->S;   // (stream, even rows | odd rows): see the kernel's cell order
         const int fblocks = (cells + kCandWarps - 1) / kCandWarps;
+        // Serial mode, at most two CTAs per SM: K2 is launched as a programmatic dependent of K1 all the same —
+        // it is scheduled while the GEMM runs, fetches its per-request parameters and waits on the device
+        // (griddepcontrol.wait) for the GEMM's results, which hides its launch latency (config 2: 17.6 vs 18.1,
+        // config 3: 69.6 vs 70.1 us/step).  A dependent grid's CTAs become resident wherever an SM has room,
+        // i.e. on the few SMs the GEMM left idle or frees first, up to 16 per SM, and every cell is one latency
+        // chain: so each CTA asks for enough shared memory that no SM takes more than its even share.  Larger
+        // grids measured slower this way (config 4, 768 CTAs: 64.5 vs 59.0 us/step) and keep the plain launch.
+        const bool pdl_k2 = !overlap && !prof && c->overlap_mode != 1 && c->pdl_finalize && fblocks <= 2 * c->num_sms;
+        fp.pdl_wait = pdl_k2 ? 1 : 0;
+        if (pdl_k2) {
+            const int per_sm = std::max(1, (fblocks + c->num_sms - 1) / c->num_sms);
+            const size_t spread = (static_cast<size_t>(c->max_smem_optin) / per_sm) & ~static_cast<size_t>(1023);
+            if (spread > fsmem + 2048) fsmem = spread - 2048;
+        }
         using FinFn = void (*)(const FinalizeParams);
         const FinFn ffn = c->V <= 1024 ? cfgms_finalize_cand_kernel<1> : c->V <= 2048 ? cfgms_finalize_cand_kernel<2>
                         : c->V <= 4096 ? cfgms_finalize_cand_kernel<4> : cfgms_finalize_cand_kernel<8>;
@@ -440,8 +460,12 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         lc.attrs = attr;
-        lc.numAttrs = (overlap && !prof) ? 1 : 0;
-        if (cudaLaunchKernelEx(&lc, ffn, fp) != cudaSuccess) return CFGMS_ERR_CUDA;
+        lc.numAttrs = ((overlap && !prof) || pdl_k2) ? 1 : 0;
+        if (cudaLaunchKernelEx(&lc, ffn, fp) != cudaSuccess) {
+            // K1 is already enqueued: leave no armed counters behind for the next step's K2
+            if (c->ready) cudaMemsetAsync(c->ready, 0, static_cast<size_t>(c->ready_words - 32) * sizeof(int), st);
+            return CFGMS_ERR_CUDA;
+        }
     } else {
         const dim3 fgrid(c->S, a->R);
         const size_t fsmem = static_cast<size_t>(c->V) * 8;

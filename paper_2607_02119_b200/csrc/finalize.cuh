@@ -63,6 +63,9 @@ struct FinalizeParams {
     int* err;                 // sticky error word
     int BN, num_row_blocks, ready_target;
     int poll_ns;              // sleep between two polls of a ready counter
+    int pdl_wait;             // 1: launched as a programmatic dependent of K1 WITHOUT ready counters: the per-request
+                              //    parameters are fetched while K1 still runs, then griddepcontrol.wait orders
+                              //    everything K1 wrote (z, candidates) before the first read of it
     int stream_base, stream_stride;   // global stream of local stream i = base + i * stride (stream-sharded heads)
 #ifdef CFGMS_TRACE
     unsigned long long* trace;
@@ -141,7 +144,7 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
         // frame count is fixed the moment stream 0 emits the end-of-audio token; other streams of this
         // step are unaffected (tau < tau + i), so nothing in this launch depends on what is written here
         constexpr int kUnset = 2147483647;
-        int F = p.n_frames ? p.n_frames[r] : kUnset;
+        int F = p.n_frames ? __ldcg(p.n_frames + r) : kUnset;
         if (F == kUnset && p.eos_token >= 0 && token == p.eos_token) F = tau;
         if (p.step_next_out) p.step_next_out[r] = tau + 1;
         if (p.n_frames_next_out) p.n_frames_next_out[r] = F;
@@ -149,7 +152,7 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
     }
     if (i == p.S - 1 && (p.frame_out || p.frame_index_out)) {
         const int f = tau - p.S + 1;
-        const bool done = f >= 0 && (p.n_frames == nullptr || f < p.n_frames[r]) && p.delayed && p.T_cap >= p.S;
+        const bool done = f >= 0 && (p.n_frames == nullptr || f < __ldcg(p.n_frames + r)) && p.delayed && p.T_cap >= p.S;
         if (p.frame_index_out) {
             p.frame_index_out[r] = done ? f : -1;
             if (pm >= 0) p.frame_index_out[pm] = -1;
@@ -158,7 +161,7 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
             int32_t* fr = p.frame_out + static_cast<size_t>(r) * p.S;
             const int32_t* ring = p.delayed + static_cast<size_t>(r) * p.T_cap * p.S;
             for (int j = 0; j < p.S; ++j)
-                fr[j] = !done ? p.pad_token : j == p.S - 1 ? token : ring[static_cast<size_t>((f + j) % p.T_cap) * p.S + j];
+                fr[j] = !done ? p.pad_token : j == p.S - 1 ? token : __ldcg(ring + static_cast<size_t>((f + j) % p.T_cap) * p.S + j);
             if (pm >= 0)
                 for (int j = 0; j < p.S; ++j) p.frame_out[static_cast<size_t>(pm) * p.S + j] = p.pad_token;
         }
@@ -481,14 +484,18 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     const int r = in_range ? r_raw : 0;
     // every per-request parameter is requested here, before any of them is used: one L2 round trip for
     // all of them instead of one per dependent use (row r is always a readable row)
+    // (step / n_frames may be the previous step's step_next_out / n_frames_next_out: read through L2)
     const int pm = p.pair_map[r];
-    const int tau = p.step[r];
-    const int F_req = p.n_frames ? p.n_frames[r] : 2147483647;
+    const int tau = __ldcg(p.step + r);
+    const int F_req = p.n_frames ? __ldcg(p.n_frames + r) : 2147483647;
     const float temp = p.temp[r];
     const int tk_raw = p.top_k[r];
     const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
     const int ft = forced_token(p, r, i);
     const bool valid = in_range && !(pm >= 0 && (r & 1));   // a companion row is written by its cond row
+    // Serial mode, small grids: this grid was scheduled while the head GEMM was still running (programmatic
+    // dependent launch); its launch latency and the parameter fetch above are behind it when the GEMM ends.
+    if (p.pdl_wait) pdl_wait_primary();
 
     const int V = p.V;
     const int G = V >> 5;            // chunks of this cell

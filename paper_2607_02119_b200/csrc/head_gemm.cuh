@@ -314,7 +314,10 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         // Let the finalize grid (K2, launched with programmatic stream serialization) be scheduled beside
         // this one: it consumes finished (stream, row block) groups through p.ready while the GEMM is still
         // running.  Only after the wait above: K2 of THIS step must not poll the ready counters before K2
-        // of the previous step has re-armed them.
+        // of the previous step has re-armed them.  (Transitive ordering is assumed here, as everywhere a kernel
+        // chains programmatic launches: K2's inputs from the PREVIOUS step's K2 — the delay ring, the
+        // device-resident request state — are visible to it because this thread saw that grid complete before
+        // it allowed K2 to start; K2 reads them through L2 (ld.cg), never through a possibly stale L1 line.)
         pdl_launch_dependents();
         const int ew = warp - kCtrlWarps;
         const int quarter = warp & 3;             // TMEM lane quarter this warp may read
