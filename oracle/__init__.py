@@ -60,6 +60,13 @@ def lib():
         L.oracle_feedback.argtypes = [C.c_void_p, C.c_void_p] + [C.c_int32] * 4 + [C.c_void_p]
         L.oracle_advance_state.restype = C.c_int32
         L.oracle_advance_state.argtypes = [C.c_int32] * 6 + [C.c_void_p, C.c_void_p]
+        L.oracle_phase_advance.restype = C.c_int32
+        L.oracle_phase_advance.argtypes = [C.c_int32] * 9 + [C.c_void_p] * 3
+        L.oracle_step_phase.restype = C.c_int
+        L.oracle_step_phase.argtypes = ([C.c_void_p] * 3 + [C.c_int32] * 4 + [C.c_void_p] * 4 + [C.c_uint64]
+                                        + [C.c_void_p] * 3 + [C.c_int32, C.c_double, C.c_void_p, C.c_int64]
+                                        + [C.c_void_p] * 6 + [C.c_int32] + [C.c_void_p] * 3 + [C.c_int32, C.c_void_p, C.c_int32,
+                                                                                                C.c_void_p])
         L.oracle_logits_row.restype = None
         L.oracle_logits_row.argtypes = [C.c_void_p] * 3 + [C.c_int32] * 5 + [C.c_void_p]
         L.oracle_cfg_merge.restype = None
@@ -288,3 +295,64 @@ def advance_state(tau: int, F: int, tok0: int, eos: int, S: int):
     tn, fn = C.c_int32(), C.c_int32()
     done = lib().oracle_advance_state(int(tau), int(F), int(tok0), int(eos), int(S), F_UNSET, C.byref(tn), C.byref(fn))
     return int(tn.value), int(fn.value), bool(done)
+
+
+# ---- widening W6: per-request phase state machine (readings C28-C32) ----
+PHASE_TEXT, PHASE_TRANSITION, PHASE_AUDIO, PHASE_DONE = 0, 1, 2, 3
+
+
+def phase_advance(phase: int, pos: int, F: int, tok0: int, modality_audio: bool, n_bridge: int, eos: int, S: int):
+    """One transition of the phase state machine -> (phase_next, pos_next, F_next, done)."""
+    pn, qn, fn = C.c_int32(), C.c_int32(), C.c_int32()
+    done = lib().oracle_phase_advance(int(phase), int(pos), int(F), int(tok0), int(bool(modality_audio)), int(n_bridge),
+                                      int(eos), int(S), F_UNSET, C.byref(pn), C.byref(qn), C.byref(fn))
+    return int(pn.value), int(qn.value), int(fn.value), bool(done)
+
+
+class PhaseStepResult(StepResult):
+    __slots__ = ("modality",)
+
+
+def step_phase(heads, embeds, hidden, pair_map, w, temp, top_k, seed: int, gstep, phase, pos, V_text: int, bridge,
+               req_id=None, n_frames=None, pad_token: Optional[int] = None, cells=None, want_merged: bool = False,
+               tokens_out: Optional[np.ndarray] = None, delayed: Optional[np.ndarray] = None, tol: float = TOL,
+               hidden_is_f32: bool = False, logit_bias=None) -> PhaseStepResult:
+    """One decode step of a batch whose requests sit in different phases (oracle_step_phase).  `gstep` is the
+    request's global step (noise key); `pos` the bridging position (TRANSITION) or audio-local step (AUDIO)."""
+    h = _arr(heads, np.uint16)
+    e = _arr(embeds, np.uint16)
+    x = f32_to_bf16(hidden) if hidden_is_f32 else _arr(hidden, np.uint16)
+    S, V, d = h.shape
+    R = x.shape[0]
+    pm = _arr(pair_map, np.int32)
+    ww, tt, kk = _arr(w, np.float32), _arr(temp, np.float32), _arr(top_k, np.int32)
+    st, ph, ps = _arr(gstep, np.int32), _arr(phase, np.int32), _arr(pos, np.int32)
+    rid, nf = _arr(req_id, np.uint32), _arr(n_frames, np.int32)
+    br = np.ascontiguousarray(bridge, dtype=np.int32).reshape(-1)
+    pad = V if pad_token is None else int(pad_token)
+    if cells is None:
+        rows = [r for r in range(R) if pm[r] < 0 or r % 2 == 0]
+        cl = np.asarray([(r, i) for r in rows for i in range(S)], dtype=np.int32).reshape(-1, 2)
+    else:
+        cl = np.ascontiguousarray(cells, dtype=np.int32).reshape(-1, 2)
+    n = cl.shape[0]
+    res = PhaseStepResult()
+    res.cells = cl
+    res.tok = np.empty(n, dtype=np.int32)
+    res.margin = np.empty(n, dtype=np.float64)
+    res.flags = np.empty(n, dtype=np.int32)
+    res.modality = np.zeros(n, dtype=np.int32)
+    res.merged = np.empty((n, V), dtype=np.float64) if want_merged else None
+    res.tokens_out, res.delayed = tokens_out, delayed
+    T_cap = 0
+    if delayed is not None:
+        assert delayed.dtype == np.int32 and delayed.flags.c_contiguous and delayed.shape[0] == R
+        T_cap = delayed.shape[1]
+    lb = _arr(logit_bias, np.float64)
+    rc = lib().oracle_step_phase(_p(h), _p(e), _p(x), R, S, d, V, _p(pm), _p(ww), _p(tt), _p(kk), C.c_uint64(seed),
+                                 _p(st), _p(rid), _p(nf), pad, C.c_double(tol), _p(cl), C.c_int64(n), _p(res.tok),
+                                 _p(res.margin), _p(res.flags), _p(res.merged), _p(tokens_out), _p(delayed), T_cap, _p(lb),
+                                 _p(ph), _p(ps), int(V_text), _p(br), int(br.size), _p(res.modality))
+    if rc != 0:
+        raise ValueError(f"oracle_step_phase failed with code {rc}")
+    return res

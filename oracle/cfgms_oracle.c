@@ -42,6 +42,12 @@
  *   W4 oracle_advance_state  step counter, frame count set by end-of-audio, drained flag
  *      pin: a request driven by it to completion produces exactly interleave(grid of F frames):
  *      S(S-1)/2 PAD cells at each end, F + S - 1 steps, S - 1 PADs on the primary stream in the drain
+ *   W6 oracle_phase_advance / oracle_step_phase  per-request phase state machine: text / transition /
+ *      audio (+ drain) / done, vocabulary regions, CFG merge only in the audio phase, modality by argmax over
+ *      the regions
+ *      pin: hand-written traces of the transition function; an all-audio batch == oracle_step_ex bit-exactly;
+ *      text-phase cells == a non-CFG run restricted to the text region (merge bypassed); region sampling ==
+ *      -inf masking of the complement (W2's pinned mask); modality vs numpy argmax
  */
 #include <math.h>
 #include <stdint.h>
@@ -167,10 +173,13 @@ static int cmp_desc(const void* a, const void* b) {
 }
 
 /* Returns the token. margin = best - second best perturbed score inside keep (+inf if alone).
- * flags: ORC_GREEDY / ORC_CLOSE / ORC_BOUNDARY.  thr_out (nullable) = top-k threshold on z. */
-int32_t oracle_sample_cell(const double* M, int32_t V, float temp, int32_t top_k, uint64_t seed,
-                           uint32_t req_id, int32_t tau, int32_t stream, double tol,
-                           double* margin_out, int32_t* flags_out, double* thr_out) {
+ * flags: ORC_GREEDY / ORC_CLOSE / ORC_BOUNDARY.  thr_out (nullable) = top-k threshold on z.
+ * M holds the V logits of tokens v_off .. v_off + V - 1 (a vocabulary REGION, widening W6; v_off = 0
+ * for a whole sub-vocabulary): the returned token is region-local, the noise of entry v is keyed by
+ * its global token id v_off + v. */
+static int32_t sample_cell_region(const double* M, int32_t V, int32_t v_off, float temp, int32_t top_k, uint64_t seed,
+                                  uint32_t req_id, int32_t tau, int32_t stream, double tol,
+                                  double* margin_out, int32_t* flags_out, double* thr_out) {
     int32_t flags = 0;
     double margin = INFINITY;
     int32_t tok = 0;
@@ -193,7 +202,7 @@ int32_t oracle_sample_cell(const double* M, int32_t V, float temp, int32_t top_k
         int first = 1;
         for (int32_t v = 0; v < V; ++v) {                                    /* O8 */
             if (z[v] >= thr) {
-                s[v] = z[v] + oracle_gumbel(seed, req_id, tau, stream, v);
+                s[v] = z[v] + oracle_gumbel(seed, req_id, tau, stream, v_off + v);
                 if (first || s[v] > s[tok]) { tok = v; first = 0; }
             }
         }
@@ -203,7 +212,7 @@ int32_t oracle_sample_cell(const double* M, int32_t V, float temp, int32_t top_k
         if (z[tok] < thr + tol && k < V) flags |= ORC_BOUNDARY;
         for (int32_t v = 0; v < V; ++v) {
             if (z[v] < thr && z[v] >= thr - tol) {
-                double sv = z[v] + oracle_gumbel(seed, req_id, tau, stream, v);
+                double sv = z[v] + oracle_gumbel(seed, req_id, tau, stream, v_off + v);
                 if (sv >= s[tok] - tol) flags |= ORC_BOUNDARY;
             }
         }
@@ -213,6 +222,12 @@ int32_t oracle_sample_cell(const double* M, int32_t V, float temp, int32_t top_k
     if (margin_out) *margin_out = margin;
     if (flags_out) *flags_out = flags;
     return tok;
+}
+
+int32_t oracle_sample_cell(const double* M, int32_t V, float temp, int32_t top_k, uint64_t seed,
+                           uint32_t req_id, int32_t tau, int32_t stream, double tol,
+                           double* margin_out, int32_t* flags_out, double* thr_out) {
+    return sample_cell_region(M, V, 0, temp, top_k, seed, req_id, tau, stream, tol, margin_out, flags_out, thr_out);
 }
 
 /* ---- O2: batch layout contract ------------------------------------------------------------ */
@@ -429,4 +444,149 @@ void oracle_sample_sweep(const double* M, int32_t V, float temp, int32_t top_k, 
                                              NULL, NULL, NULL);
             counts[tok] += 1;
         }
+}
+
+
+/* ---- Widening W6 — per-request phase state machine (readings C28-C32 of DESIGN.md) ----
+ * "a per-request phase state machine enforced via dynamic vocabulary masking ... a text phase restricted
+ * to text tokens, a transition phase injecting deterministic bridging tokens to condition audio
+ * generation, and an audio phase activating all S streams ... terminating the audio phase initiates a
+ * drain sub-phase that emits S-1 padding tokens ... dynamically inferring the active modality directly
+ * from the model's unmasked output distribution (i.e., the argmax over the disjoint vocabulary regions)"
+ * and "this CFG merge operates only during the audio phase; it bypasses modality-switching
+ * tokens".
+ *
+ * C28 the PRIMARY stream (stream 0) is the one that carries text: its V logits cover the disjoint regions
+ *     [0, V_text) = text tokens and [V_text, V) = its audio codes (and the end-of-audio id); streams >= 1
+ *     are audio only.  "Dynamic vocabulary masking" = the phase selects the region a cell may sample from.
+ * C29 TEXT: only stream 0 samples, from the text region, from the CONDITIONAL row's logits alone (no merge);
+ *     streams >= 1 emit PAD.  The modality the model asks for is the region of argmax_v of the UNMASKED
+ *     logits of stream 0 (lowest v on ties); when it is the audio region, the request leaves the text phase
+ *     AFTER this step (the step's token is still the text token it sampled).
+ * C30 TRANSITION: stream 0 emits the deterministic bridging tokens bridge[0..n_bridge-1], one per step,
+ *     streams >= 1 emit PAD, nothing is sampled; then the audio phase starts with audio-local step 0.
+ * C31 AUDIO: rows a1-a4 of the hot path with the audio-local step tau_a (delay pattern, frame count, ring
+ *     slot), stream 0 restricted to its audio region; the end-of-audio token on stream 0 fixes the frame count
+ *     (W4) and the drain runs S-1 more steps; then DONE (every stream PAD, state frozen).
+ * C32 the noise is keyed by the request's GLOBAL step (monotone over all phases), never by the phase-local
+ *     position, so no two steps of a request share noise.
+ *
+ * One transition.  `pos` = bridging tokens emitted so far (TRANSITION) or the audio-local step tau_a (AUDIO).
+ * tok0 = stream 0's token of this step; modality_audio = C29's inference (only read in TEXT).
+ * Returns 1 iff the request is DONE after this step. */
+#define ORC_PHASE_TEXT 0
+#define ORC_PHASE_TRANSITION 1
+#define ORC_PHASE_AUDIO 2
+#define ORC_PHASE_DONE 3
+
+int32_t oracle_phase_advance(int32_t phase, int32_t pos, int32_t F, int32_t tok0, int32_t modality_audio,
+                             int32_t n_bridge, int32_t eos, int32_t S, int32_t unset,
+                             int32_t* phase_next, int32_t* pos_next, int32_t* F_next) {
+    int32_t pn = phase, qn = pos, Fn = F;
+    if (phase == ORC_PHASE_TEXT) {
+        qn = 0;
+        if (modality_audio) pn = n_bridge > 0 ? ORC_PHASE_TRANSITION : ORC_PHASE_AUDIO;
+    } else if (phase == ORC_PHASE_TRANSITION) {
+        if (pos + 1 >= n_bridge) { pn = ORC_PHASE_AUDIO; qn = 0; }
+        else qn = pos + 1;
+    } else if (phase == ORC_PHASE_AUDIO) {
+        int32_t tn;
+        int32_t drained = oracle_advance_state(pos, F, tok0, eos, S, unset, &tn, &Fn);   /* W4 with tau = tau_a */
+        qn = tn;
+        if (drained) pn = ORC_PHASE_DONE;
+    }
+    *phase_next = pn; *pos_next = qn; *F_next = Fn;
+    return pn == ORC_PHASE_DONE ? 1 : 0;
+}
+
+/* One decode step of a batch whose requests sit in different phases.  Arguments as oracle_step_ex, plus
+ *   phase, pos    int32 [R], read at the request-owning row (C29-C31)
+ *   gstep         int32 [R] the request's global step: keys the noise (C32)
+ *   V_text        size of stream 0's text region (C28), 0 <= V_text <= V
+ *   bridge        int32 [n_bridge] bridging tokens (C30)
+ * n_frames [R] (nullable = unset) is relative to the audio-local step.  Per evaluated cell j: tok_out,
+ * margin_out, flags_out, merged_out (the logits the cell sampled from BEFORE the region restriction: cond-only
+ * in TEXT, merged in AUDIO; zeros where nothing was sampled).  Per evaluated cell of stream 0 additionally
+ * modality_out[j] = 1 when C29's argmax lies in the audio region (0 elsewhere).  tokens_out / delayed as in
+ * oracle_step_ex, except that only AUDIO-phase cells write the delayed buffer, at slot tau_a mod T_cap. */
+int oracle_step_phase(const uint16_t* heads, const uint16_t* embeds, const uint16_t* hidden,
+                      int32_t R, int32_t S, int32_t d, int32_t V,
+                      const int32_t* pair_map, const float* w, const float* temp, const int32_t* top_k,
+                      uint64_t seed, const int32_t* gstep, const uint32_t* req_id, const int32_t* n_frames,
+                      int32_t pad_token, double tol,
+                      const int32_t* cells, int64_t n_cells,
+                      int32_t* tok_out, double* margin_out, int32_t* flags_out, double* merged_out,
+                      int32_t* tokens_out, int32_t* delayed, int32_t T_cap,
+                      const double* logit_bias,
+                      const int32_t* phase, const int32_t* pos, int32_t V_text,
+                      const int32_t* bridge, int32_t n_bridge, int32_t* modality_out) {
+    if (R <= 0 || S <= 0 || d <= 0 || V <= 0 || !cells || !phase || !pos || V_text < 0 || V_text > V) return ORACLE_ERR_ARG;
+    int rc = oracle_check_pair_map(pair_map, R);
+    if (rc != ORACLE_OK) return rc;
+    for (int64_t j = 0; j < n_cells; ++j) {
+        int32_t c = cells[2 * j], i = cells[2 * j + 1];
+        if (c < 0 || c >= R || i < 0 || i >= S || (pair_map[c] >= 0 && c % 2 == 1)) return ORACLE_ERR_ARG;
+        if (phase[c] == ORC_PHASE_TRANSITION && (pos[c] < 0 || pos[c] >= n_bridge)) return ORACLE_ERR_ARG;
+    }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t j = 0; j < n_cells; ++j) {
+        int32_t c = cells[2 * j], i = cells[2 * j + 1];
+        int32_t u = pair_map[c];
+        int32_t ph = phase[c], q = pos[c];
+        uint32_t rid = req_id ? req_id[c] : (uint32_t)c;
+        int32_t tok = pad_token, flags = ORC_INACTIVE, modality = 0;
+        double margin = INFINITY;
+        int sample = 0, merge = 0;
+        int32_t lo = 0, hi = V;
+        if (ph == ORC_PHASE_TEXT) {                                   /* C29 */
+            if (i == 0) { sample = 1; merge = 0; lo = 0; hi = V_text; }
+        } else if (ph == ORC_PHASE_TRANSITION) {                      /* C30 */
+            if (i == 0) { tok = bridge[q]; flags = ORC_FORCED; }
+        } else if (ph == ORC_PHASE_AUDIO) {                           /* C31: O5 with tau_a */
+            int active = (i <= q) && (n_frames == NULL || q - i < n_frames[c]);
+            if (active) { sample = 1; merge = 1; lo = i == 0 ? V_text : 0; hi = V; }
+        }
+        if (merged_out) memset(merged_out + (size_t)j * V, 0, sizeof(double) * (size_t)V);
+        if (sample) {
+            double* Lc = (double*)malloc(sizeof(double) * (size_t)V * 3);
+            double* Lu = Lc + V;
+            double* M = Lc + 2 * (size_t)V;
+            oracle_logits_row(heads, embeds, hidden, S, d, V, c, i, Lc);                          /* O3 */
+            if (merge && u >= 0) {
+                oracle_logits_row(heads, embeds, hidden, S, d, V, u, i, Lu);
+                oracle_cfg_merge(Lc, Lu, (double)w[c], V, M);                                     /* O4, audio phase only */
+            } else {
+                memcpy(M, Lc, sizeof(double) * (size_t)V);
+            }
+            if (logit_bias)
+                for (int32_t v = 0; v < V; ++v) M[v] += logit_bias[(size_t)i * V + v];
+            if (ph == ORC_PHASE_TEXT) {                                                           /* C29: unmasked argmax */
+                int32_t am = 0;
+                for (int32_t v = 1; v < V; ++v) if (M[v] > M[am]) am = v;
+                modality = am >= V_text ? 1 : 0;
+            }
+            flags = 0;
+            if (hi > lo) {
+                tok = lo + sample_cell_region(M + lo, hi - lo, lo, temp[c], top_k[c], seed, rid, gstep[c], i, tol,
+                                              &margin, &flags, NULL);                              /* O6-O8 on the region */
+            } else {
+                tok = pad_token; flags = ORC_INACTIVE;      /* empty region: nothing to sample */
+            }
+            if (merged_out) memcpy(merged_out + (size_t)j * V, M, sizeof(double) * (size_t)V);
+            free(Lc);
+        }
+        if (tok_out) tok_out[j] = tok;
+        if (margin_out) margin_out[j] = margin;
+        if (flags_out) flags_out[j] = flags;
+        if (modality_out) modality_out[j] = modality;
+        if (tokens_out) {                                                                         /* O9 */
+            tokens_out[(size_t)c * S + i] = tok;
+            if (u >= 0) tokens_out[(size_t)u * S + i] = tok;
+        }
+        if (delayed && T_cap > 0 && ph == ORC_PHASE_AUDIO) {
+            int32_t slot = ((q % T_cap) + T_cap) % T_cap;
+            delayed[((size_t)c * T_cap + slot) * S + i] = tok;
+        }
+    }
+    return ORACLE_OK;
 }
