@@ -84,7 +84,9 @@ typedef struct {
                               sample exactly what one unsharded context samples; the caller gathers
                               tokens_out [R][S_local] of all shards (<= 32 KB per step).  stride <= 0
                               means unsharded (base 0, stride 1).  frame_out needs an unsharded context */
-    int32_t reserved[1];
+    int32_t global_streams; /* stream-sharded heads: the number of streams of the WHOLE head (the drain of a
+                               request ends S_global - 1 steps after its last frame); 0 = this context's S.
+                               A sharded context needs it to write step_next_out / n_frames_next_out / done_out */
 } cfgms_config;
 
 /*
@@ -154,7 +156,34 @@ typedef struct {
                                  end-of-audio token appears; n_frames == NULL reads as UNSET)       */
     int32_t* done_out;        /* [R] 1 when the request is fully drained after this step
                                  (tau + 1 >= frames + S - 1), else 0                               */
+    /* per-request phase state machine on the device; see cfgms_set_phase_table.
+       phase == NULL: every request is in the audio phase with audio-local step = step[r] (the plain path). */
+    const int32_t* phase;     /* [R] cfgms_phase of the request, read at the cond / unpaired row              */
+    const int32_t* phase_pos; /* [R] TRANSITION: bridging tokens emitted so far; AUDIO: the audio-local step
+                                 tau_a (delay pattern, frame count, ring slot); ignored otherwise.  With
+                                 phases, step[r] is the request's GLOBAL step and only keys the noise, and
+                                 n_frames counts audio-local steps.  Required when `phase` is given; force_token
+                                 must then be NULL (the transition phase is the forced-token mechanism)  */
+    int32_t* phase_next_out;  /* [R] nullable: the phase after this step                                    */
+    int32_t* phase_pos_next_out; /* [R] nullable: phase_pos after this step.  Feed both back as phase / phase_pos
+                                 (two buffers, alternating), together with step_next_out / n_frames_next_out  */
+    int32_t* modality_out;    /* [R] nullable: 1 when a TEXT-phase request's unmasked stream-0 logits peak in the
+                                 audio region (the inference that ends its text phase), else 0                */
 } cfgms_step_args;
+
+/* Phases of a request.  The PRIMARY stream (global stream 0) carries text: its V logits cover
+ * the disjoint regions [0, V_text) = text tokens and [V_text, V) = its audio codes (and the end-of-audio id);
+ * the other streams are audio only.  "Dynamic vocabulary masking" = the phase selects the region sampled from.
+ *   TEXT        only stream 0 samples, from the text region, from the CONDITIONAL row's logits alone (the CFG
+ *               merge "operates only during the audio phase"); the other streams emit the pad
+ *               token.  The modality the model asks for is the region of the argmax of stream 0's unmasked
+ *               logits; when it is the audio region the request moves on after this step.
+ *   TRANSITION  stream 0 emits the deterministic bridging tokens, one per step; nothing is sampled.
+ *   AUDIO       the hot path as described above with the audio-local step tau_a = phase_pos; stream 0 is
+ *               restricted to its audio region; the end-of-audio token (eos_token) on stream 0 fixes the frame
+ *               count and the drain runs S - 1 more steps; then
+ *   DONE        every stream emits the pad token, the state is frozen, done_out = 1.                        */
+typedef enum { CFGMS_PHASE_TEXT = 0, CFGMS_PHASE_TRANSITION = 1, CFGMS_PHASE_AUDIO = 2, CFGMS_PHASE_DONE = 3 } cfgms_phase;
 
 #define CFGMS_FRAMES_UNSET 2147483647 /* n_frames value meaning "no frame count yet" (no drain)   */
 
@@ -188,6 +217,14 @@ int cfgms_step_host(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stre
  * per-token bias once, on `cuda_stream`; costs nothing per step.  Not retained.
  */
 int cfgms_set_logit_bias(cfgms_ctx* ctx, const float* bias, void* cuda_stream);
+
+/*
+ * cfgms_set_phase_table — configuration of the phase state machine: V_text = size of the text
+ * region of stream 0 (0 <= V_text <= V; a multiple of 32 when V is, so that a region is whole candidate chunks),
+ * bridge_tokens = HOST int32 [n_bridge], 0 <= n_bridge <= 16, the deterministic bridging tokens of the
+ * transition phase (copied).  Takes effect for steps enqueued afterwards.  Errors: ARG, SHAPE.
+ */
+int cfgms_set_phase_table(cfgms_ctx* ctx, int32_t V_text, const int32_t* bridge_tokens, int32_t n_bridge);
 
 /*
  * cfgms_feedback — autoregressive feedback aggregation ("the input representation

@@ -28,7 +28,7 @@ STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR
 EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
            "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats",
-           "cfgms_set_logit_bias", "cfgms_feedback"]
+           "cfgms_set_logit_bias", "cfgms_feedback", "cfgms_set_phase_table"]
 
 
 class CfgmsError(RuntimeError):
@@ -40,7 +40,7 @@ class CfgmsError(RuntimeError):
 class cfgms_config(C.Structure):
     _fields_ = [("max_rows", C.c_int32), ("pad_token", C.c_int32), ("flags", C.c_uint32),
                 ("row_tile", C.c_int32), ("max_stages", C.c_int32), ("stream_base", C.c_int32),
-                ("stream_stride", C.c_int32), ("reserved", C.c_int32 * 1)]
+                ("stream_stride", C.c_int32), ("global_streams", C.c_int32)]
 
 
 class cfgms_step_args(C.Structure):
@@ -50,7 +50,9 @@ class cfgms_step_args(C.Structure):
                 ("tokens_out", C.c_void_p), ("delayed", C.c_void_p), ("T_cap", C.c_int32),
                 ("logits_out", C.c_void_p), ("force_token", C.c_void_p), ("frame_out", C.c_void_p),
                 ("frame_index_out", C.c_void_p), ("eos_token", C.c_int32), ("step_next_out", C.c_void_p),
-                ("n_frames_next_out", C.c_void_p), ("done_out", C.c_void_p)]
+                ("n_frames_next_out", C.c_void_p), ("done_out", C.c_void_p), ("phase", C.c_void_p),
+                ("phase_pos", C.c_void_p), ("phase_next_out", C.c_void_p), ("phase_pos_next_out", C.c_void_p),
+                ("modality_out", C.c_void_p)]
 
 
 class cfgms_info(C.Structure):
@@ -95,6 +97,8 @@ def _lib():
         L.cfgms_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cfgms_set_logit_bias.restype = C.c_int
         L.cfgms_set_logit_bias.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.cfgms_set_phase_table.restype = C.c_int
+        L.cfgms_set_phase_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]
         L.cfgms_feedback.restype = C.c_int
         L.cfgms_feedback.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.cfgms_overlap_stats.restype = C.c_int
@@ -146,7 +150,7 @@ class Context:
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
                  cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0,
                  force_overlap: bool = False, stream_base: int = 0, stream_stride: int = 0,
-                 no_pdl_finalize: bool = False):
+                 no_pdl_finalize: bool = False, global_streams: int = 0):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -158,6 +162,7 @@ class Context:
         cfg.row_tile = int(row_tile)
         cfg.max_stages = int(max_stages)
         cfg.stream_base, cfg.stream_stride = int(stream_base), int(stream_stride)   # stream-sharded heads
+        cfg.global_streams = int(global_streams)
         if pad_token is not None:
             cfg.pad_token = int(pad_token)
             cfg.flags |= CFGMS_CFG_PAD_TOKEN
@@ -194,7 +199,8 @@ class Context:
 
     def _args(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
               logits_out, dev: str, force_token=None, frame_out=None, frame_index_out=None, eos_token=-1,
-              step_next_out=None, n_frames_next_out=None, done_out=None) -> cfgms_step_args:
+              step_next_out=None, n_frames_next_out=None, done_out=None, phase=None, phase_pos=None,
+              phase_next_out=None, phase_pos_next_out=None, modality_out=None) -> cfgms_step_args:
         R = int(hidden.shape[0])
         _check(hidden, "hidden", (torch.bfloat16, torch.float32), dev, R * self.d)
         if hidden.dim() != 2 or hidden.shape[1] != self.d:
@@ -232,15 +238,21 @@ class Context:
             _check(t, name, torch.int32, "cuda", R, optional=True)
         a.eos_token = int(eos_token)
         a.step_next_out, a.n_frames_next_out, a.done_out = _ptr(step_next_out), _ptr(n_frames_next_out), _ptr(done_out)
+        for t, name in ((phase, "phase"), (phase_pos, "phase_pos"), (phase_next_out, "phase_next_out"),
+                        (phase_pos_next_out, "phase_pos_next_out"), (modality_out, "modality_out")):
+            _check(t, name, torch.int32, "cuda", R, optional=True)
+        a.phase, a.phase_pos = _ptr(phase), _ptr(phase_pos)
+        a.phase_next_out, a.phase_pos_next_out, a.modality_out = _ptr(phase_next_out), _ptr(phase_pos_next_out), _ptr(modality_out)
         return a
 
     def step(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
              delayed=None, logits_out=None, stream=None, force_token=None, frame_out=None,
-             frame_index_out=None, eos_token=-1, step_next_out=None, n_frames_next_out=None, done_out=None) -> None:
+             frame_index_out=None, eos_token=-1, step_next_out=None, n_frames_next_out=None, done_out=None,
+             phase=None, phase_pos=None, phase_next_out=None, phase_pos_next_out=None, modality_out=None) -> None:
         """cfgms_step: device tensors, enqueue only."""
         a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
                        logits_out, "cuda", force_token, frame_out, frame_index_out, eos_token, step_next_out,
-                       n_frames_next_out, done_out)
+                       n_frames_next_out, done_out, phase, phase_pos, phase_next_out, phase_pos_next_out, modality_out)
         rc = _lib().cfgms_step(self._h, C.byref(a), _stream_ptr(stream))
         if rc != 0:
             raise CfgmsError(rc, "cfgms_step")
@@ -278,6 +290,14 @@ class Context:
         bias.masked_fill_(col >= torch.tensor(sizes, device=dev).unsqueeze(1), float("-inf"))
         self.set_logit_bias(bias, stream=stream)
         return bias
+
+    def set_phase_table(self, V_text: int, bridge_tokens=()) -> None:
+        """cfgms_set_phase_table: text region [0, V_text) of stream 0 and the transition phase's bridging tokens."""
+        br = [int(x) for x in bridge_tokens]
+        arr = (C.c_int32 * max(len(br), 1))(*br)
+        rc = _lib().cfgms_set_phase_table(self._h, int(V_text), arr, len(br))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_set_phase_table")
 
     def feedback(self, tokens: torch.Tensor, emb: torch.Tensor, x_out: Optional[torch.Tensor] = None,
                  stream=None) -> torch.Tensor:

@@ -45,6 +45,9 @@ struct cfgms_ctx {
     int device = 0, num_sms = 0;
     int max_rows = 0, pad_token = 0, row_tile_override = 0, max_stages = 0;
     int stream_base = 0, stream_stride = 1;   // stream-sharded heads: global stream of local stream i
+    int S_total = 0;                  // streams of the whole head (== S unless stream-sharded); 0 = unknown (sharded, not given)
+    int V_text = 0, n_bridge = 0;     // phase state machine (cfgms_set_phase_table)
+    int32_t bridge[16] = {0};
     int poll_ns = 2000;       // K2's sleep between polls of a ready counter: 1-4 us measured ~2.4 % faster than 50-200 ns at config 5
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     bool pdl_finalize = true;         // serial mode: launch a small K2 grid as a programmatic dependent of K1
@@ -137,6 +140,11 @@ int validate_step(const cfgms_ctx* c, const cfgms_step_args* a) {
     if (a->delayed && a->T_cap < 1) return CFGMS_ERR_ARG;
     if ((a->frame_out || a->frame_index_out) && (!a->delayed || a->T_cap < c->S)) return CFGMS_ERR_ARG;
     if ((a->frame_out || a->frame_index_out) && (c->stream_base != 0 || c->stream_stride != 1)) return CFGMS_ERR_ARG;   // a frame needs every stream
+    // the drain of a request ends S_global - 1 steps after its last frame: a shard must know S_global
+    if ((a->step_next_out || a->n_frames_next_out || a->done_out || a->phase_next_out || a->phase_pos_next_out) && c->S_total == 0)
+        return CFGMS_ERR_ARG;
+    if (a->phase && (!a->phase_pos || a->force_token)) return CFGMS_ERR_ARG;
+    if (!a->phase && (a->phase_pos || a->phase_next_out || a->phase_pos_next_out || a->modality_out)) return CFGMS_ERR_ARG;
     return CFGMS_OK;
 }
 
@@ -187,6 +195,9 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     c->max_stages = (cfg && cfg->max_stages >= 2) ? cfg->max_stages : kMaxStages;
     if (cfg && cfg->stream_stride > 0) { c->stream_base = cfg->stream_base; c->stream_stride = cfg->stream_stride; }
     if (c->stream_base < 0) { delete c; return CFGMS_ERR_ARG; }
+    const bool sharded = c->stream_base != 0 || c->stream_stride != 1;
+    c->S_total = (cfg && cfg->global_streams > 0) ? cfg->global_streams : (sharded ? 0 : S);
+    if (c->S_total != 0 && c->S_total < c->stream_base + (S - 1) * c->stream_stride + 1) { delete c; return CFGMS_ERR_ARG; }
     c->pair_mode = (cfg && (cfg->flags & CFGMS_CFG_SINGLE_CTA)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_CTA_PAIR)) ? 2 : 0;
     if (c->row_tile_override < 0 || c->row_tile_override > kMaxBN || (c->row_tile_override % 64) != 0) {
         delete c;
@@ -348,7 +359,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     int stages = static_cast<int>((static_cast<uint32_t>(c->max_smem_optin) - 1024 - GemmSmemLayout::misc_bytes()) / stage_bytes);
     stages = std::max(2, std::min(stages, std::min(kMaxStages, c->max_stages)));
     gp.stages = stages;
-    gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp;
+    gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp; gp.phase = a->phase;
     gp.bias = c->bias; gp.z = c->z; gp.tap = a->logits_out; gp.err = c->err;
     gp.cand_val = c->cand_val; gp.cand_src = c->cand_src;
     const int workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
@@ -421,6 +432,11 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.err = c->err;
     fp.BN = BN; fp.num_row_blocks = nrb;
     fp.stream_base = c->stream_base; fp.stream_stride = c->stream_stride;
+    fp.S_total = c->S_total > 0 ? c->S_total : c->S;
+    fp.phase = a->phase; fp.phase_pos = a->phase_pos;
+    fp.phase_next_out = a->phase_next_out; fp.phase_pos_next_out = a->phase_pos_next_out; fp.modality_out = a->modality_out;
+    fp.V_text = c->V_text; fp.n_bridge = c->n_bridge;
+    std::memcpy(fp.bridge, c->bridge, sizeof(fp.bridge));
     fp.poll_ns = c->poll_ns;
     fp.pdl_wait = 0;
 #ifdef CFGMS_TRACE
@@ -548,6 +564,16 @@ int cfgms_set_logit_bias(cfgms_ctx* c, const float* bias, void* cuda_stream) {
     cfgms_bias_fold_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->bias_base, bias, c->bias, c->NT);
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.launches_total += 1;
+    return CFGMS_OK;
+}
+
+int cfgms_set_phase_table(cfgms_ctx* c, int32_t V_text, const int32_t* bridge_tokens, int32_t n_bridge) {
+    if (!c || V_text < 0 || V_text > c->V || n_bridge < 0 || n_bridge > 16 || (n_bridge > 0 && !bridge_tokens)) return CFGMS_ERR_ARG;
+    // on the candidate path a vocabulary region must be whole 32-token chunks
+    if (c->use_cand && (V_text % 32) != 0) return CFGMS_ERR_SHAPE;
+    c->V_text = V_text;
+    c->n_bridge = n_bridge;
+    for (int j = 0; j < 16; ++j) c->bridge[j] = j < n_bridge ? bridge_tokens[j] : 0;
     return CFGMS_OK;
 }
 

@@ -67,6 +67,16 @@ struct FinalizeParams {
                               //    parameters are fetched while K1 still runs, then griddepcontrol.wait orders
                               //    everything K1 wrote (z, candidates) before the first read of it
     int stream_base, stream_stride;   // global stream of local stream i = base + i * stride (stream-sharded heads)
+    int S_total;              // streams of the whole head (== S unless stream-sharded): ends the drain
+    // per-request phase state machine (include/cfgms.h); phase == nullptr: plain path
+    const int32_t* phase;        // [R]
+    const int32_t* phase_pos;    // [R]
+    int32_t* phase_next_out;     // [R] nullable
+    int32_t* phase_pos_next_out; // [R] nullable
+    int32_t* modality_out;       // [R] nullable
+    int V_text;                  // text region of stream 0: [0, V_text)
+    int n_bridge;
+    int32_t bridge[16];          // bridging tokens of the transition phase
 #ifdef CFGMS_TRACE
     unsigned long long* trace;
 #endif
@@ -128,31 +138,87 @@ __device__ __forceinline__ int forced_token(const FinalizeParams& p, int r, int 
     return p.force_token ? p.force_token[static_cast<size_t>(r) * p.S + i] : -1;
 }
 
+// What one (request, stream) cell does at this step.  Plain path (p.phase == nullptr): the request is in the
+// audio phase with audio-local step tau_a = step[r].  With the phase state machine (include/cfgms.h):
+//   TEXT        stream 0 samples from the text region [0, V_text), the other streams pad; want_modality
+//   TRANSITION  stream 0 emits bridge[pos], the other streams pad
+//   AUDIO       delay pattern on tau_a = pos; stream 0 samples from its audio region [V_text, V)
+//   DONE        pad
+constexpr int kPhaseText = 0, kPhaseTransition = 1, kPhaseAudio = 2, kPhaseDone = 3;
+struct CellPlan {
+    int phase;          // kPhaseAudio on the plain path
+    int pos;            // phase_pos (== tau_a in the audio phase)
+    int gstep;          // step[r]: keys the noise
+    int tau_a;          // audio-local step (delay pattern, ring slot, frames); meaningful in the audio phase
+    int lo, hi;         // vocabulary region the cell samples from
+    int token;          // what an inactive cell emits (pad or a bridging token)
+    bool sample;        // the cell draws a token from [lo, hi)
+    bool want_modality; // TEXT phase, stream 0: also find the region of the unmasked argmax
+};
+__device__ __forceinline__ CellPlan plan_cell(const FinalizeParams& p, int r, int gi, int gstep, int F_req) {
+    CellPlan c;
+    c.phase = kPhaseAudio; c.pos = gstep; c.gstep = gstep; c.tau_a = gstep;
+    c.lo = 0; c.hi = p.V; c.token = p.pad_token; c.sample = false; c.want_modality = false;
+    if (p.phase) {
+        c.phase = __ldcg(p.phase + r);
+        c.pos = __ldcg(p.phase_pos + r);
+        c.tau_a = c.pos;
+    }
+    if (c.phase == kPhaseAudio) {
+        c.sample = (gi <= c.tau_a) && (c.tau_a - gi < F_req);
+        if (p.phase && gi == 0) c.lo = p.V_text;
+    } else if (c.phase == kPhaseText) {
+        if (gi == 0) { c.sample = true; c.want_modality = true; c.hi = p.V_text; }
+    } else if (c.phase == kPhaseTransition) {
+        if (gi == 0 && c.pos >= 0 && c.pos < p.n_bridge) c.token = p.bridge[c.pos];
+    }
+    if (c.hi <= c.lo) c.sample = false;        // empty region: nothing to sample, the cell pads
+    return c;
+}
+
 // Rows a4 of the hot path, by ONE thread per cell: token to the row and its companion
 // (PAPER.md:93), delayed-layout cell.  The thread of the LAST stream also emits
 // the frame that completes at this step: f = tau - S + 1, frame[i] = ring[(f + i) mod
 // T_cap][i]; streams i < S - 1 were written by earlier steps' launches, stream S - 1 is `token`.
-__device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i, int pm, int tau, int token) {
+// The thread of the PRIMARY stream's cell advances the request's state (phase, position, frame count).
+__device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i, int pm, const CellPlan& cp, int token,
+                                           int modality) {
+    const int tau = cp.tau_a;
+    const bool audio = cp.phase == kPhaseAudio;
     p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
     if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
-    if (p.delayed) {
+    if (p.delayed && audio) {          // only audio-phase tokens belong to the codebook matrix
         const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
         p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
     }
-    if (global_stream(p, i) == 0 && (p.step_next_out || p.n_frames_next_out || p.done_out)) {
+    if (global_stream(p, i) == 0) {
         // request state for the next step, by the thread of the PRIMARY stream's cell: the
         // frame count is fixed the moment stream 0 emits the end-of-audio token; other streams of this
         // step are unaffected (tau < tau + i), so nothing in this launch depends on what is written here
         constexpr int kUnset = 2147483647;
         int F = p.n_frames ? __ldcg(p.n_frames + r) : kUnset;
-        if (F == kUnset && p.eos_token >= 0 && token == p.eos_token) F = tau;
-        if (p.step_next_out) p.step_next_out[r] = tau + 1;
+        int phase_next = cp.phase, pos_next = cp.pos;
+        if (cp.phase == kPhaseText) {
+            pos_next = 0;
+            if (modality) phase_next = p.n_bridge > 0 ? kPhaseTransition : kPhaseAudio;
+        } else if (cp.phase == kPhaseTransition) {
+            if (cp.pos + 1 >= p.n_bridge) { phase_next = kPhaseAudio; pos_next = 0; }
+            else pos_next = cp.pos + 1;
+        } else if (audio) {
+            if (F == kUnset && p.eos_token >= 0 && token == p.eos_token) F = tau;
+            pos_next = tau + 1;
+            if (F != kUnset && tau + 1 >= F + p.S_total - 1) phase_next = kPhaseDone;
+        }
+        if (p.step_next_out) p.step_next_out[r] = cp.gstep + 1;
         if (p.n_frames_next_out) p.n_frames_next_out[r] = F;
-        if (p.done_out) p.done_out[r] = (F != kUnset && tau + 1 >= F + p.S - 1) ? 1 : 0;
+        if (p.done_out) p.done_out[r] = phase_next == kPhaseDone ? 1 : 0;
+        if (p.phase_next_out) p.phase_next_out[r] = phase_next;
+        if (p.phase_pos_next_out) p.phase_pos_next_out[r] = pos_next;
+        if (p.modality_out) p.modality_out[r] = modality;
     }
     if (i == p.S - 1 && (p.frame_out || p.frame_index_out)) {
         const int f = tau - p.S + 1;
-        const bool done = f >= 0 && (p.n_frames == nullptr || f < __ldcg(p.n_frames + r)) && p.delayed && p.T_cap >= p.S;
+        const bool done = audio && f >= 0 && (p.n_frames == nullptr || f < __ldcg(p.n_frames + r)) && p.delayed && p.T_cap >= p.S;
         if (p.frame_index_out) {
             p.frame_index_out[r] = done ? f : -1;
             if (pm >= 0) p.frame_index_out[pm] = -1;
@@ -264,10 +330,12 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
     const int pm = p.pair_map[r];
     if (pm >= 0 && (r & 1)) return;  // companion row: its cond row writes both
 
-    const int tau = p.step[r];
     const int gi = global_stream(p, i);
-    bool active = (gi <= tau) && (p.n_frames == nullptr || tau - gi < p.n_frames[r]);
-    int token = p.pad_token;
+    const CellPlan cp = plan_cell(p, r, gi, __ldcg(p.step + r), p.n_frames ? __ldcg(p.n_frames + r) : 2147483647);
+    const int tau = cp.gstep;          // keys the noise
+    bool active = cp.sample;
+    int token = cp.token;
+    int modality = 0;
     if (active) {
         const int ft = forced_token(p, r, i);
         if (ft >= 0) { token = ft; active = false; }
@@ -275,6 +343,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
 
     if (active) {
         const int V = p.V;
+        const int Vr = cp.hi - cp.lo;      // size of the vocabulary region this cell samples from
         uint32_t* cand_key = dyn;
         int* cand_idx = reinterpret_cast<int*>(dyn + V);
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
@@ -284,10 +353,25 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
             const int v = j * kFinThreads + tid;
             key[j] = v < V ? float_key(__ldg(zr + v)) : 0u;
         }
+        if (cp.want_modality) {
+            // the modality the model asks for: region of the argmax of the UNMASKED logits (lowest token on ties)
+            BestSV m = {-INFINITY, 0x7fffffff};
+#pragma unroll
+            for (int j = 0; j < EPT; ++j)
+                if (key[j] != 0u) best_update(m, key_float(key[j]), j * kFinThreads + tid);
+            m = block_argmax(m, red_s, red_v);
+            if (tid == 0) modality = m.v >= p.V_text ? 1 : 0;
+            __syncthreads();               // red_s / red_v are reused by the sampling argmax below
+        }
+#pragma unroll
+        for (int j = 0; j < EPT; ++j) {    // dynamic vocabulary masking: tokens outside the region do not exist
+            const int v = j * kFinThreads + tid;
+            if (v < cp.lo || v >= cp.hi) key[j] = 0u;
+        }
         const float temp = p.temp[r];
         const int tk = p.top_k[r];
         const bool greedy = (tk == 1) || (temp == 0.f);
-        const bool filter = !greedy && tk > 0 && tk < V;
+        const bool filter = !greedy && tk > 0 && tk < Vr;
         const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
         BestSV best = {-INFINITY, 0x7fffffff};
 
@@ -351,7 +435,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
 #pragma unroll
             for (int j = 0; j < EPT; ++j) {
                 const int v = j * kFinThreads + tid;
-                if (v < V) {
+                if (key[j] != 0u) {
                     float s = key_float(key[j]);
                     if (!greedy) s += gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v);
                     best_update(best, s, v);
@@ -361,7 +445,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
         best = block_argmax(best, red_s, red_v);
         token = best.v;
     }
-    if (tid == 0) write_cell(p, r, i, pm, tau, token);
+    if (tid == 0) write_cell(p, r, i, pm, cp, token, modality);
 }
 
 // Fallback for V > 256 * 32: keys in shared memory, radix select over all of them.
@@ -376,26 +460,36 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
     const int i = blockIdx.x, r = blockIdx.y, tid = threadIdx.x;
     const int pm = p.pair_map[r];
     if (pm >= 0 && (r & 1)) return;
-    const int tau = p.step[r];
     const int gi = global_stream(p, i);
-    bool active = (gi <= tau) && (p.n_frames == nullptr || tau - gi < p.n_frames[r]);
-    int token = p.pad_token;
+    const CellPlan cp = plan_cell(p, r, gi, __ldcg(p.step + r), p.n_frames ? __ldcg(p.n_frames + r) : 2147483647);
+    const int tau = cp.gstep;          // keys the noise
+    bool active = cp.sample;
+    int token = cp.token;
+    int modality = 0;
     if (active) {
         const int ft = forced_token(p, r, i);
         if (ft >= 0) { token = ft; active = false; }
     }
     if (active) {
         const int V = p.V;
+        const int Vr = cp.hi - cp.lo;
         const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
         for (int v = tid; v < V; v += kFinThreads) dyn[v] = float_key(__ldg(zr + v));
         __syncthreads();
+        if (cp.want_modality) {            // region of the argmax of the unmasked logits
+            BestSV m = {-INFINITY, 0x7fffffff};
+            for (int v = tid; v < V; v += kFinThreads) best_update(m, key_float(dyn[v]), v);
+            m = block_argmax(m, red_s, red_v);
+            if (tid == 0) modality = m.v >= p.V_text ? 1 : 0;
+            __syncthreads();
+        }
         const float temp = p.temp[r];
         const int tk = p.top_k[r];
         const bool greedy = (tk == 1) || (temp == 0.f);
         uint32_t thr_key = 0u;
-        if (!greedy && tk > 0 && tk < V) {
+        if (!greedy && tk > 0 && tk < Vr) {
             if (tid < 32) {
-                const uint32_t t = warp_radix_select(SmemKeys{dyn}, V, tk, hist, tid);
+                const uint32_t t = warp_radix_select(SmemKeys{dyn + cp.lo}, Vr, tk, hist, tid);
                 if (tid == 0) thr_key_s = t;
             }
             __syncthreads();
@@ -403,7 +497,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
         }
         const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
         BestSV best = {-INFINITY, 0x7fffffff};
-        for (int v = tid; v < V; v += kFinThreads) {
+        for (int v = cp.lo + tid; v < cp.hi; v += kFinThreads) {
             const uint32_t k = dyn[v];
             if (k >= thr_key) {
                 float s = key_float(k);
@@ -414,7 +508,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
         best = block_argmax(best, red_s, red_v);
         token = best.v;
     }
-    if (tid == 0) write_cell(p, r, i, pm, tau, token);
+    if (tid == 0) write_cell(p, r, i, pm, cp, token, modality);
 }
 
 
@@ -486,8 +580,11 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     // all of them instead of one per dependent use (row r is always a readable row)
     // (step / n_frames may be the previous step's step_next_out / n_frames_next_out: read through L2)
     const int pm = p.pair_map[r];
-    const int tau = __ldcg(p.step + r);
+    const int gstep = __ldcg(p.step + r);
     const int F_req = p.n_frames ? __ldcg(p.n_frames + r) : 2147483647;
+    const int gi = global_stream(p, i);
+    const CellPlan cp = plan_cell(p, r, gi, gstep, F_req);   // phase, vocabulary region, audio-local step
+    const int tau = cp.gstep;                                 // keys the noise
     const float temp = p.temp[r];
     const int tk_raw = p.top_k[r];
     const uint32_t req = p.req_id ? p.req_id[r] : static_cast<uint32_t>(r);
@@ -497,19 +594,23 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     // dependent launch); its launch latency and the parameter fetch above are behind it when the GEMM ends.
     if (p.pdl_wait) pdl_wait_primary();
 
-    const int V = p.V;
-    const int G = V >> 5;            // chunks of this cell
+    // The cell samples from the vocabulary region [cp.lo, cp.hi) of its stream (the whole sub-vocabulary on the
+    // plain path; whole 32-token chunks always: the host checks the phase table).  Everything below works in
+    // region-local tokens and chunks; `tok0` turns them back into tokens of the stream.
+    const int tok0 = cp.lo;
+    const int V = cp.hi - cp.lo;     // tokens of the region
+    const int G = V >> 5;            // chunks of the region
     const int E = G * 4;             // emitted values
-    const int cap = cand_list_cap(V);
-    int* hist = reinterpret_cast<int*>(dyn + static_cast<size_t>(warp) * cand_warp_words(V));
+    const int cap = cand_list_cap(p.V);
+    int* hist = reinterpret_cast<int*>(dyn + static_cast<size_t>(warp) * cand_warp_words(p.V));
     uint32_t* small = reinterpret_cast<uint32_t*>(hist + 256);
     int* misc = reinterpret_cast<int*>(small + 32);
     uint32_t* list_key = reinterpret_cast<uint32_t*>(misc + 8);
     int* list_v = reinterpret_cast<int*>(list_key + cap);
 
-    const int gi = global_stream(p, i);
-    bool active = valid && (gi <= tau) && (tau - gi < F_req);
-    int token = p.pad_token;
+    bool active = valid && cp.sample;
+    int token = cp.token;
+    int modality = 0;
     if (active && ft >= 0) { token = ft; active = false; }
     if (valid && p.ready) {
         // Wait until K1 has written every tile of this (stream, row block): the acquire pairs with the
@@ -533,8 +634,22 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     }
     CFGMS_K2_MARK(2);      // parameters in, readiness wait over
     if (active) {
-        const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V;
-        const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * V) >> 5;
+        const float* zr = p.z + static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * p.V + tok0;
+        const size_t chunk0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * p.V + tok0) >> 5;
+        if (cp.want_modality) {
+            // The modality the model asks for: region of the argmax of stream 0's UNMASKED logits.
+            // Every chunk's first emitted value is its exact maximum (lowest token among equals), so the row's
+            // argmax is the best of the chunk maxima — over ALL chunks of the stream, not only the region's.
+            const size_t row0 = (static_cast<size_t>(r) * p.NT + static_cast<size_t>(i) * p.V) >> 5;
+            BestSV m = {-INFINITY, 0x7fffffff};
+            for (int c = lane; c < (p.V >> 5); c += 32) {
+                const float top = __ldcg(p.cand_val + (row0 + c) * 4);
+                const uint32_t off = __ldcg(p.cand_src + row0 + c) & 31u;
+                best_update(m, top, c * 32 + static_cast<int>(off));
+            }
+            m = warp_argmax(m);
+            modality = m.v >= p.V_text ? 1 : 0;
+        }
         const bool greedy = (tk_raw == 1) || (temp == 0.f);
         const bool filter = !greedy && tk_raw > 0 && tk_raw < V;
         const int tk = greedy ? 1 : tk_raw;   // greedy = exact top-1 (ties: lowest token), no noise
@@ -655,7 +770,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                         if (pred) {
                             const int pos = n_list + __popc(b & ((1u << lane) - 1u));
                             list_key[pos] = key[j][e];
-                            list_v[pos] = c * 32 + static_cast<int>((src[j] >> (8 * e)) & 31u);
+                            list_v[pos] = tok0 + c * 32 + static_cast<int>((src[j] >> (8 * e)) & 31u);
                         }
                         n_list += __popc(b);
                     }
@@ -687,7 +802,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                                 if (pred) {
                                     const int pos = n_list + __popc(b & ((1u << lane) - 1u));
                                     list_key[pos] = k32;
-                                    list_v[pos] = cc[u] * 32 + lane;
+                                    list_v[pos] = tok0 + cc[u] * 32 + lane;
                                 }
                                 n_list += __popc(b);
                             }
@@ -739,7 +854,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                     for (int v = lane; v < V; v += 32) {
                         const float zv = __ldcg(zr + v);
                         if (float_key(zv) >= thr_full)
-                            best_update(best, greedy ? zv + 0.0f : zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
+                            best_update(best, greedy ? zv + 0.0f : zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, tok0 + v), tok0 + v);
                     }
                 }
             }
@@ -750,14 +865,14 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
             for (int v = lane; v < V; v += 32) {
                 const float zv = __ldcg(zr + v);
                 if (float_key(zv) >= thr_full)
-                    best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
+                    best_update(best, zv + 0.0f + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, tok0 + v), tok0 + v);
             }
         }
         best = warp_argmax(best);
         token = best.v;
         CFGMS_K2_MARK(7);          // noise drawn, argmax done
     }
-    if (valid && lane == 0) write_cell(p, r, i, pm, tau, token);
+    if (valid && lane == 0) write_cell(p, r, i, pm, cp, token, modality);
     CFGMS_K2_MARK(8);
     if (p.ready) {
         // the last CTA to finish re-arms the counters for the next step's K1 (which starts after this grid)

@@ -67,6 +67,7 @@ struct GemmParams {
     const int32_t* pair_map;
     const float* w;
     const float* temp;
+    const int32_t* phase; // nullable [R]: request phase (include/cfgms.h); the CFG merge runs in the audio phase only
     const float* bias;   // [NT]
     float* z;            // [R][NT]
     float* tap;          // nullable [R][NT]
@@ -105,7 +106,9 @@ __device__ __forceinline__ void make_slot_coef(const GemmParams& p, int r0, Slot
     const float t0 = p.temp[r0];
     const float it0 = t0 == 0.f ? 1.f : 1.f / t0;
     if (pm0 == r1 && pm1 == r0) {                       // (cond, uncond) pair: Eq. 1
-        const float w = p.w[r0];
+        // "this CFG merge operates only during the audio phase; it bypasses modality-switching
+        // tokens": outside the audio phase the request's logits are its conditional row's (w = 1 in Eq. 1)
+        const float w = (p.phase && __ldcg(p.phase + r0) != 2 /* CFGMS_PHASE_AUDIO */) ? 1.f : p.w[r0];
         a.c00 = w * it0; a.c01 = (1.f - w) * it0; a.d0 = it0; a.kind = 1;
         b.m00 = w; b.m01 = 1.f - w;
     } else if (pm0 == -1 && pm1 == -1) {                // two unpaired rows
