@@ -99,42 +99,55 @@ class Runner:
 
     cta_pair = None   # tuning override (--cta-pair): None = library default
 
-    def __init__(self, cfg: int, dev, cfg_off: bool = False, rank: int = 0, n_ranks: int = 1):
+    def __init__(self, cfg: int, dev, cfg_off: bool = False, rank: int = 0, n_ranks: int = 1, shard_streams: bool = False):
         import torch
         import paper_2607_02119_b200 as pkg
-        from paper_2607_02119_b200.dist_utils import shard_request_ids
+        from paper_2607_02119_b200 import dist_utils
         import workloads
         self.torch = torch
         wl = workloads.make_config(cfg, cfg_off=cfg_off)
-        if rank:  # every rank serves its own requests: distinct hidden states and request ids
-            g = torch.Generator().manual_seed(1000 + rank)
-            wl.hidden_pool = torch.randn(wl.hidden_pool.shape, generator=g).to(wl.hidden_pool.dtype)
-        first, _ = shard_request_ids(rank, n_ranks, wl.n_req)
-        wl.req_id = wl.req_id + first
+        self.shard_streams = shard_streams
+        self.S_local = wl.S
         self.wl, self.dev = wl, dev
         cu = lambda t: None if t is None else t.to(dev)
-        self.heads, self.embeds = cu(wl.heads), cu(wl.embeds)
-        self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), cta_pair=Runner.cta_pair)
+        if shard_streams:
+            # stream-sharded heads (W5): every rank sees all rows and all requests, holds the
+            # head slices of streams {rank, rank + N, ...} and exchanges tokens from inside the finalize kernel
+            base, stride, self.S_local = dist_utils.stream_shard(rank, n_ranks, wl.S)
+            self.heads, self.embeds = cu(wl.heads[base::stride].contiguous()), cu(wl.embeds[base::stride].contiguous())
+            self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), cta_pair=Runner.cta_pair,
+                                   stream_base=base, stream_stride=stride, global_streams=wl.S)
+            dist_utils.connect_stream_exchange(self.ctx, rank, n_ranks)
+        else:
+            if rank:  # every rank serves its own requests: distinct hidden states and request ids
+                g = torch.Generator().manual_seed(1000 + rank)
+                wl.hidden_pool = torch.randn(wl.hidden_pool.shape, generator=g).to(wl.hidden_pool.dtype)
+            first, _ = dist_utils.shard_request_ids(rank, n_ranks, wl.n_req)
+            wl.req_id = wl.req_id + first
+            self.heads, self.embeds = cu(wl.heads), cu(wl.embeds)
+            self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), cta_pair=Runner.cta_pair)
         self.pool = cu(wl.hidden_pool)
         self.pair_map, self.w, self.temp, self.top_k = cu(wl.pair_map), cu(wl.w), cu(wl.temp), cu(wl.top_k)
         self.req_id, self.n_frames = cu(wl.req_id), cu(wl.n_frames)
-        self.tokens = torch.zeros((wl.R, wl.S), dtype=torch.int32, device=dev)
-        self.delayed = torch.full((wl.R, wl.T, wl.S), wl.pad_token, dtype=torch.int32, device=dev)
-        self.grid = torch.zeros((wl.R, wl.T - wl.S + 1, wl.S), dtype=torch.int32, device=dev)
+        self.tokens = torch.zeros((wl.R, self.S_local), dtype=torch.int32, device=dev)
+        self.delayed = torch.full((wl.R, wl.T, self.S_local), wl.pad_token, dtype=torch.int32, device=dev)
+        self.grid = None if shard_streams else torch.zeros((wl.R, wl.T - wl.S + 1, wl.S), dtype=torch.int32, device=dev)
         # request-local steps of every engine iteration, resident on the device
         ts = torch.arange(wl.T, dtype=torch.int32).unsqueeze(1) + wl.offset.unsqueeze(0)
         self.steps_dev = ts.contiguous().to(dev)
-        self.flops_per_step = 2.0 * wl.R * wl.S * wl.d * wl.V
+        self.flops_per_step = 2.0 * wl.R * self.S_local * wl.d * wl.V      # of THIS rank
         # algorithmic bytes per step: weights once, hidden once, merged
         # logits written and read once (fp32), tokens + delayed cells
-        self.bytes_per_step = (2.0 * wl.S * wl.d * wl.V + 2.0 * wl.R * wl.d + 2 * 4.0 * wl.n_req * wl.S * wl.V
-                               + 4.0 * wl.S * (wl.R + wl.n_req))
+        self.bytes_per_step = (2.0 * self.S_local * wl.d * wl.V + 2.0 * wl.R * wl.d + 2 * 4.0 * wl.n_req * self.S_local * wl.V
+                               + 4.0 * self.S_local * (wl.R + wl.n_req))
 
     def step(self, t: int):
         wl = self.wl
         self.ctx.step(self.pool[t % self.pool.shape[0]], self.pair_map, self.w, self.temp, self.top_k, wl.seed,
                       self.steps_dev[t % wl.T], self.tokens, req_id=self.req_id, n_frames=self.n_frames,
                       delayed=self.delayed)
+        if self.shard_streams:
+            self.ctx.exchange_wait(wl.R)     # every rank's tokens of this step are in this rank's gather buffer
 
     def deinterleave(self):
         self.ctx.deinterleave(self.delayed, self.grid)
@@ -295,9 +308,13 @@ class Runner:
         pool = [pin(wl.hidden_pool[j]) for j in range(wl.hidden_pool.shape[0])]
         pm, w, temp, tk, rid, nf = map(pin, (wl.pair_map, wl.w, wl.temp, wl.top_k, wl.req_id, wl.n_frames))
         steps = [pin((wl.offset + t).to(torch.int32)) for t in range(min(wl.T, warmup + K))]
-        tok = torch.zeros((wl.R, wl.S), dtype=torch.int32).pin_memory()
-        call = lambda t: self.ctx.step_host(pool[t % len(pool)], pm, w, temp, tk, wl.seed, steps[t % len(steps)], tok,
-                                            req_id=rid, n_frames=nf, delayed=self.delayed)
+        tok = torch.zeros((wl.R, self.S_local), dtype=torch.int32).pin_memory()
+
+        def call(t):
+            self.ctx.step_host(pool[t % len(pool)], pm, w, temp, tk, wl.seed, steps[t % len(steps)], tok,
+                               req_id=rid, n_frames=nf, delayed=self.delayed)
+            if self.shard_streams:
+                self.ctx.exchange_wait(wl.R)
         for t in range(warmup):
             call(t)
         torch.cuda.synchronize()
@@ -382,11 +399,11 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def workload_config(wl, cfg, launch):
+def workload_config(wl, cfg, launch, parallelism=None):
     return {"workload": f"BASELINE.json configs[{cfg - 1}] '{wl.name}': {wl.n_req} requests in {wl.R} rows "
                         f"({int((wl.pair_map >= 0).sum()) // 2} CFG pairs), d={wl.d}, S={wl.S}, V={wl.V}, T={wl.T}",
             "rows": wl.R, "requests": wl.n_req, "d": wl.d, "S": wl.S, "V": wl.V, "T": wl.T,
-            "parallelism": "request-sharded replicas (no data-path collective)", "launch": launch}
+            "parallelism": parallelism or "request-sharded replicas (no data-path collective)", "launch": launch}
 
 
 def main():
@@ -394,14 +411,20 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=None, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip ratio / other configs / cold-L2 legs")
+    ap.add_argument("--shard", default="requests", choices=["requests", "streams"],
+                    help="multi-GPU sharding: 'requests' = independent replicas (default, weak scaling); 'streams' = every rank "
+                         "holds the head slices of streams {rank, rank + N, ...}, all ranks see all rows, tokens are exchanged "
+                         "by the finalize kernel through peer-mapped memory (strong scaling of the weight stream; default config 3)")
     ap.add_argument("--cta-pair", default="auto", choices=["auto", "on", "off"],
                     help="tuning: force the CTA-pair (cta_group::2) or the one-CTA head GEMM")
     args = ap.parse_args()
     Runner.cta_pair = {"auto": None, "on": True, "off": False}[args.cta_pair]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.config is None:
+        args.config = 3 if args.shard == "streams" else 5
     if args.impl == "reference":
         run_reference(args)
         return
@@ -418,12 +441,17 @@ def main():
     peaks = load_peaks()
     K, W = args.steps, args.warmup
 
-    main_r = Runner(args.config, dev, rank=rank, n_ranks=world)
+    sharded = args.shard == "streams"
+    main_r = Runner(args.config, dev, rank=rank, n_ranks=world, shard_streams=sharded)
     wl = main_r.wl
     K = min(K, 4096)
     sampler = ClockSampler(local_rank)
-    elapsed_ms = main_r.time_graph(K, W, with_deint=True, barrier=lambda: dist_utils.barrier(dev), sampler=sampler)
-    value, worst_ms = dist_utils.whole_job_rate(float(wl.n_req) * K, elapsed_ms, dev)
+    elapsed_ms = main_r.time_graph(K, W, with_deint=not sharded, barrier=lambda: dist_utils.barrier(dev), sampler=sampler)
+    if sharded:   # every rank works on the SAME requests: the job's frames are counted once, the time is the slowest rank's
+        worst_ms = dist_utils.max_over_ranks(elapsed_ms, dev)
+        value = float(wl.n_req) * K / (worst_ms * 1e-3)
+    else:
+        value, worst_ms = dist_utils.whole_job_rate(float(wl.n_req) * K, elapsed_ms, dev)
     info = main_r.ctx.info()
     gemm_us, fin_us = main_r.time_kernels(min(K, 512), 3)
     us_per_step = 1e3 * worst_ms / K
@@ -444,20 +472,28 @@ def main():
                     roofline_us_per_step=1e6 * max(t_tensor, t_hbm), step_frac=max(t_tensor, t_hbm) * 1e6 / us_per_step,
                     frac_of_sustained_peak=(roof["achieved"] / peaks["tflops_sustained"]) if roof["bound"] == "tensor" else None)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": worst_ms / K, "us_per_step": us_per_step, "higher_is_better": True, "scaling": "weak",
+                "ms_per_step": worst_ms / K, "us_per_step": us_per_step, "higher_is_better": True,
+                "scaling": "strong" if sharded else "weak",
                 "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": dict(workload_config(wl, args.config, f"one CUDA graph of {K} cfgms_step + 1 cfgms_deinterleave"),
+                "config": dict(workload_config(wl, args.config, (f"one CUDA graph of {K} x (cfgms_step + cfgms_exchange_wait)" if sharded else
+                                                                  f"one CUDA graph of {K} cfgms_step + 1 cfgms_deinterleave"),
+                                               parallelism=(f"stream-sharded heads: {main_r.S_local} of {wl.S} streams per rank, token all-gather by "
+                                                            "peer stores from the finalize kernel (no collective on the data path)") if sharded else None),
                                l2="inputs larger than L2: head weights %.0f MiB + hidden pool %.0f MiB + logits %.0f MiB" % (
                                    wl.heads.numel() * 2 / 2 ** 20, wl.hidden_pool.numel() * wl.hidden_pool.element_size() / 2 ** 20,
                                    wl.n_req * wl.S * wl.V * 4 / 2 ** 20),
                                row_tile=info["row_tile"], row_blocks=info["row_blocks"], gemm_grid=info["gemm_grid"],
                                pipeline_stages=info["pipeline_stages"], cta_pair=bool(info["cta_pair"])),
-                "clocks": sampler.summary(), "gpu_launches": int(info["launches_last_step"] * K + 1), "roofline": roof}
+                "clocks": sampler.summary(), "gpu_launches": int((info["launches_last_step"] + (1 if sharded else 0)) * K + (0 if sharded else 1)),
+                "roofline": roof}
 
     # end-to-end through the host-buffer entry point (every rank, max over ranks)
     Ke = min(K, 64)
     dt_e2e, h2d, d2h = main_r.time_e2e(Ke, 3)
-    e2e_value, _ = dist_utils.whole_job_rate(float(wl.n_req) * Ke, dt_e2e * 1e3, dev)
+    if sharded:
+        e2e_value = float(wl.n_req) * Ke / dist_utils.max_over_ranks(dt_e2e, dev)
+    else:
+        e2e_value, _ = dist_utils.whole_job_rate(float(wl.n_req) * Ke, dt_e2e * 1e3, dev)
     if rank == 0:
         line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                        "us_per_step": 1e6 * dt_e2e / Ke, "api": "cfgms_step_host (pinned host buffers, sync per step)"}
@@ -465,7 +501,7 @@ def main():
     if rank == 0 and world == 1:
         cb, _, _ = oracle_sample(wl)
         line["cpu_baseline"] = cb
-        if not args.no_extras:
+        if not args.no_extras and not sharded:
             wd = main_r.time_widenings(50)
             wd["feedback_frac_of_hbm_peak"] = wd["feedback_gbs"] / peaks["hbm_gbs"]
             line["widenings"] = wd

@@ -227,6 +227,38 @@ int cfgms_set_logit_bias(cfgms_ctx* ctx, const float* bias, void* cuda_stream);
 int cfgms_set_phase_table(cfgms_ctx* ctx, int32_t V_text, const int32_t* bridge_tokens, int32_t n_bridge);
 
 /*
+ * Stream-sharded heads: the token exchange as a device-side operation (decode is memory-bound,
+ * so dividing the weight stream over G GPUs is the lever; the heads are per stream).  Every rank g
+ * creates its context with stream_base = g, stream_stride = G, global_streams = S_global and sees all rows; the
+ * step's one exchange is an all-gather of the sampled tokens, done BY THE FINALIZE KERNEL: the thread that
+ * writes a cell's token also stores it into every rank's gather buffer int32 [max_rows][S_global] (peer-mapped
+ * memory, NVLink), and the grid's last CTA then raises one flag per destination.  No collective library call is
+ * on the data path.  The gather buffer is double-buffered by step parity: a rank can run at most one step ahead of
+ * a peer (its next step needs that peer's tokens), so the half it overwrites has been consumed everywhere.
+ *   cfgms_exchange_create       allocates this rank's block (gather buffer + flags) with cudaMalloc; returns its
+ *                               CUDA IPC handle (64 bytes, nullable) and/or its device address (nullable).  All ranks
+ *                               must use the same max_rows and S_global.
+ *   cfgms_exchange_connect      peer_bases: HOST array [world] of the ranks' block addresses AS VALID IN THIS
+ *                               PROCESS (entry [rank] is ignored): for peers in the same process or memory
+ *                               mapped by other means; from then on every cfgms_step of this context scatters.
+ *   cfgms_exchange_connect_ipc  handles: HOST [world][64] bytes, every rank's IPC handle in rank order; opens the
+ *                               peers' blocks (closed at cfgms_destroy) and connects.
+ *   cfgms_exchange_wait         enqueues a one-CTA kernel that waits (bounded, 2 s -> CFGMS_ERR_TIMEOUT) until the
+ *                               tokens of every rank's current step have landed in this rank's gather buffer, then
+ *                               copies rows [0, R) of the step's half to the buffer cfgms_exchange_tokens returns;
+ *                               kernels enqueued after it on the stream may read that.  Call it exactly once per
+ *                               step.  Epochs are counted on the device: CUDA-graph replay is fine.
+ *   cfgms_exchange_tokens       *tokens_all_out = the gathered tokens of the last waited step, DEVICE int32
+ *                               [max_rows][S_global] (owned by the context).
+ * Errors: ARG (no global stream count, exchange already created / not created), NOMEM, CUDA.
+ */
+int cfgms_exchange_create(cfgms_ctx* ctx, int32_t world, int32_t rank, void* ipc_handle_out, void** base_out);
+int cfgms_exchange_connect(cfgms_ctx* ctx, void* const* peer_bases);
+int cfgms_exchange_connect_ipc(cfgms_ctx* ctx, const void* handles);
+int cfgms_exchange_wait(cfgms_ctx* ctx, int32_t R, void* cuda_stream);
+int cfgms_exchange_tokens(cfgms_ctx* ctx, const int32_t** tokens_all_out);
+
+/*
  * cfgms_feedback — autoregressive feedback aggregation ("the input representation
  * at each step aggregates the embeddings of these previously generated tokens"):
  *     x_out[r][k] = bf16_rne( sum_{i < S} emb[i][tokens[r][i]][k] )     (fp32 sum, i ascending)

@@ -28,7 +28,8 @@ STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR
 EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
            "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats",
-           "cfgms_set_logit_bias", "cfgms_feedback", "cfgms_set_phase_table"]
+           "cfgms_set_logit_bias", "cfgms_feedback", "cfgms_set_phase_table", "cfgms_exchange_create",
+           "cfgms_exchange_connect", "cfgms_exchange_connect_ipc", "cfgms_exchange_wait", "cfgms_exchange_tokens"]
 
 
 class CfgmsError(RuntimeError):
@@ -97,6 +98,16 @@ def _lib():
         L.cfgms_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cfgms_set_logit_bias.restype = C.c_int
         L.cfgms_set_logit_bias.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.cfgms_exchange_create.restype = C.c_int
+        L.cfgms_exchange_create.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.cfgms_exchange_connect.restype = C.c_int
+        L.cfgms_exchange_connect.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.cfgms_exchange_connect_ipc.restype = C.c_int
+        L.cfgms_exchange_connect_ipc.argtypes = [C.c_void_p, C.c_void_p]
+        L.cfgms_exchange_wait.restype = C.c_int
+        L.cfgms_exchange_wait.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+        L.cfgms_exchange_tokens.restype = C.c_int
+        L.cfgms_exchange_tokens.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
         L.cfgms_set_phase_table.restype = C.c_int
         L.cfgms_set_phase_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]
         L.cfgms_feedback.restype = C.c_int
@@ -290,6 +301,51 @@ class Context:
         bias.masked_fill_(col >= torch.tensor(sizes, device=dev).unsqueeze(1), float("-inf"))
         self.set_logit_bias(bias, stream=stream)
         return bias
+
+    # ---- stream-sharded heads: the token exchange (cfgms_exchange_*) ----
+    def exchange_create(self, world: int, rank: int):
+        """-> (64-byte CUDA IPC handle, device address) of this rank's exchange block."""
+        handle = (C.c_ubyte * 64)()
+        base = C.c_void_p()
+        rc = _lib().cfgms_exchange_create(self._h, int(world), int(rank), handle, C.byref(base))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_exchange_create")
+        self._xchg = (int(world), int(rank))
+        return bytes(handle), int(base.value)
+
+    def exchange_connect(self, peer_bases) -> None:
+        """peer_bases: the ranks' block addresses as valid in this process (same-process peers)."""
+        arr = (C.c_void_p * len(peer_bases))(*[int(b) if b else None for b in peer_bases])
+        rc = _lib().cfgms_exchange_connect(self._h, arr)
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_exchange_connect")
+
+    def exchange_connect_ipc(self, handles) -> None:
+        """handles: every rank's 64-byte IPC handle, in rank order."""
+        blob = b"".join(bytes(h) for h in handles)
+        if len(blob) != 64 * len(handles):
+            raise ValueError("every handle must be 64 bytes")
+        rc = _lib().cfgms_exchange_connect_ipc(self._h, blob)
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_exchange_connect_ipc")
+
+    def exchange_wait(self, R: int, stream=None) -> None:
+        rc = _lib().cfgms_exchange_wait(self._h, int(R), _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_exchange_wait")
+
+    def exchange_tokens(self, R: int, S_global: int) -> torch.Tensor:
+        """This rank's gather buffer as an int32 [R][S_global] tensor view (no copy; owned by the context)."""
+        p = C.c_void_p()
+        rc = _lib().cfgms_exchange_tokens(self._h, C.byref(p))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_exchange_tokens")
+        iface = {"shape": (int(R), int(S_global)), "typestr": "<i4", "data": (int(p.value), False), "version": 3,
+                 "strides": None}
+        holder = type("_CfgmsView", (), {"__cuda_array_interface__": iface})()
+        t = torch.as_tensor(holder, device=self.device)
+        t._cfgms_owner = self          # keep the context (and its block) alive
+        return t
 
     def set_phase_table(self, V_text: int, bridge_tokens=()) -> None:
         """cfgms_set_phase_table: text region [0, V_text) of stream 0 and the transition phase's bridging tokens."""

@@ -72,6 +72,16 @@ struct cfgms_ctx {
     int max_smem_optin = 0;
     HostStage hs;
     bool hs_ready = false;
+    // stream-sharded token exchange (cfgms_exchange_*): one device block [tokens | flags | state], symmetric on all ranks
+    struct {
+        int world = 0, rank = 0;
+        void* base = nullptr;                 // this rank's block (cudaMalloc: exportable through CUDA IPC)
+        size_t half_bytes = 0, latest_off = 0, flags_off = 0, state_off = 0;  // byte offsets inside every rank's block
+        void* opened[64] = {nullptr};         // peers' blocks opened through IPC (closed at destroy)
+        int32_t** d_tokens = nullptr;         // device arrays [world] of peer pointers
+        uint32_t** d_flags = nullptr;
+        bool connected = false;
+    } xc;
     bool prof_on = false;
     cudaEvent_t* prof_ev = nullptr;   // [kProfMax][3]
     int prof_n = 0;
@@ -308,6 +318,11 @@ void cfgms_destroy(cfgms_ctx* c) {
     cudaFree(c->hidden_bf16);
     cudaFree(c->err);
     cudaFree(c->ready);
+    for (int q = 0; q < 64; ++q)
+        if (c->xc.opened[q]) cudaIpcCloseMemHandle(c->xc.opened[q]);
+    cudaFree(c->xc.base);
+    cudaFree(c->xc.d_tokens);
+    cudaFree(c->xc.d_flags);
     if (c->prof_ev) {
         for (int j = 0; j < 3 * kProfMax; ++j)
             if (c->prof_ev[j]) cudaEventDestroy(c->prof_ev[j]);
@@ -436,6 +451,11 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     fp.phase = a->phase; fp.phase_pos = a->phase_pos;
     fp.phase_next_out = a->phase_next_out; fp.phase_pos_next_out = a->phase_pos_next_out; fp.modality_out = a->modality_out;
     fp.V_text = c->V_text; fp.n_bridge = c->n_bridge;
+    fp.xchg_tokens = c->xc.connected ? c->xc.d_tokens : nullptr;
+    fp.xchg_flags = c->xc.connected ? c->xc.d_flags : nullptr;
+    fp.xchg_state = c->xc.base ? reinterpret_cast<unsigned int*>(static_cast<char*>(c->xc.base) + c->xc.state_off) : nullptr;
+    fp.xchg_world = c->xc.world; fp.xchg_rank = c->xc.rank;
+    fp.xchg_half_elems = static_cast<int>(c->xc.half_bytes / sizeof(int32_t));
     std::memcpy(fp.bridge, c->bridge, sizeof(fp.bridge));
     fp.poll_ns = c->poll_ns;
     fp.pdl_wait = 0;
@@ -564,6 +584,84 @@ int cfgms_set_logit_bias(cfgms_ctx* c, const float* bias, void* cuda_stream) {
     cfgms_bias_fold_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->bias_base, bias, c->bias, c->NT);
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.launches_total += 1;
+    return CFGMS_OK;
+}
+
+int cfgms_exchange_create(cfgms_ctx* c, int32_t world, int32_t rank, void* ipc_handle_out, void** base_out) {
+    if (!c || world < 1 || world > 64 || rank < 0 || rank >= world) return CFGMS_ERR_ARG;
+    if (c->S_total == 0 || c->xc.base) return CFGMS_ERR_ARG;       // needs the global stream count; one exchange per context
+    // [half 0 | half 1 | latest | flags uint32 [64] | state]: peers write the halves and the flags only
+    c->xc.half_bytes = (static_cast<size_t>(c->max_rows) * c->S_total * sizeof(int32_t) + 255) & ~static_cast<size_t>(255);
+    c->xc.latest_off = 2 * c->xc.half_bytes;
+    c->xc.flags_off = 3 * c->xc.half_bytes;
+    c->xc.state_off = c->xc.flags_off + 256;
+    const size_t total = c->xc.state_off + 256;
+    if (cudaMalloc(&c->xc.base, total) != cudaSuccess) { c->xc.base = nullptr; return CFGMS_ERR_NOMEM; }
+    if (cudaMemset(c->xc.base, 0, total) != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->xc.world = world; c->xc.rank = rank;
+    if (ipc_handle_out) {
+        static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size is part of the ABI");
+        cudaIpcMemHandle_t h;
+        if (cudaIpcGetMemHandle(&h, c->xc.base) != cudaSuccess) return CFGMS_ERR_CUDA;
+        std::memcpy(ipc_handle_out, &h, sizeof(h));
+    }
+    if (base_out) *base_out = c->xc.base;
+    return CFGMS_OK;
+}
+
+int cfgms_exchange_connect(cfgms_ctx* c, void* const* peer_bases) {
+    if (!c || !c->xc.base || !peer_bases) return CFGMS_ERR_ARG;
+    const int world = c->xc.world;
+    int32_t* tok[64];
+    uint32_t* flg[64];
+    for (int q = 0; q < world; ++q) {
+        char* base = static_cast<char*>(q == c->xc.rank ? c->xc.base : peer_bases[q]);
+        if (!base) return CFGMS_ERR_ARG;
+        tok[q] = reinterpret_cast<int32_t*>(base);
+        flg[q] = reinterpret_cast<uint32_t*>(base + c->xc.flags_off);
+    }
+    if (!c->xc.d_tokens && (dev_alloc(&c->xc.d_tokens, 64) != CFGMS_OK || dev_alloc(&c->xc.d_flags, 64) != CFGMS_OK)) return CFGMS_ERR_NOMEM;
+    if (cudaMemcpy(c->xc.d_tokens, tok, sizeof(int32_t*) * world, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(c->xc.d_flags, flg, sizeof(uint32_t*) * world, cudaMemcpyHostToDevice) != cudaSuccess)
+        return CFGMS_ERR_CUDA;
+    c->xc.connected = true;
+    return CFGMS_OK;
+}
+
+int cfgms_exchange_connect_ipc(cfgms_ctx* c, const void* handles) {
+    if (!c || !c->xc.base || !handles) return CFGMS_ERR_ARG;
+    void* bases[64] = {nullptr};
+    for (int q = 0; q < c->xc.world; ++q) {
+        if (q == c->xc.rank) continue;
+        if (!c->xc.opened[q]) {
+            cudaIpcMemHandle_t h;
+            std::memcpy(&h, static_cast<const char*>(handles) + 64 * q, sizeof(h));
+            if (cudaIpcOpenMemHandle(&c->xc.opened[q], h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+                c->xc.opened[q] = nullptr;
+                return CFGMS_ERR_CUDA;
+            }
+        }
+        bases[q] = c->xc.opened[q];
+    }
+    return cfgms_exchange_connect(c, bases);
+}
+
+int cfgms_exchange_wait(cfgms_ctx* c, int32_t R, void* cuda_stream) {
+    if (!c || !c->xc.connected || R < 1 || R > c->max_rows) return CFGMS_ERR_ARG;
+    char* base = static_cast<char*>(c->xc.base);
+    cfgms_exchange_wait_kernel<<<1, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        reinterpret_cast<const volatile uint32_t*>(base + c->xc.flags_off),
+        reinterpret_cast<unsigned int*>(base + c->xc.state_off) + 2, c->xc.world,
+        reinterpret_cast<const int32_t*>(base), reinterpret_cast<int32_t*>(base + c->xc.latest_off),
+        static_cast<int>(c->xc.half_bytes / sizeof(int32_t)), R * c->S_total, c->err);
+    if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.launches_total += 1;
+    return CFGMS_OK;
+}
+
+int cfgms_exchange_tokens(cfgms_ctx* c, const int32_t** tokens_all_out) {
+    if (!c || !c->xc.base || !tokens_all_out) return CFGMS_ERR_ARG;
+    *tokens_all_out = reinterpret_cast<const int32_t*>(static_cast<char*>(c->xc.base) + c->xc.latest_off);
     return CFGMS_OK;
 }
 

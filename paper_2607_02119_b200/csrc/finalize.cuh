@@ -74,6 +74,17 @@ struct FinalizeParams {
     int32_t* phase_next_out;     // [R] nullable
     int32_t* phase_pos_next_out; // [R] nullable
     int32_t* modality_out;       // [R] nullable
+    // Stream-sharded heads (W5): the step's one exchange, an all-gather of the sampled
+    // tokens, done by this kernel as direct stores into every rank's gather buffer (peer-mapped memory over
+    // NVLink; this rank's own buffer included), followed by one flag per destination.  nullptr = off.
+    int32_t* const* xchg_tokens; // device array [world] of int32 [2][xchg_rows][S_total] gather buffers (rank order);
+                                 // the step that publishes epoch e writes half e & 1: a rank can run at most one
+                                 // step ahead of a peer (its next step needs that peer's tokens), so the half it
+                                 // overwrites has been consumed everywhere
+    int xchg_half_elems;         // int32 elements between the two halves (same on every rank)
+    uint32_t* const* xchg_flags; // device array [world] of uint32 [world] flag arrays: flags[q][rank] = epoch
+    unsigned int* xchg_state;    // device, this rank's: [0] CTAs done (re-armed by the last one), [1] epoch published so far
+    int xchg_world, xchg_rank;
     int V_text;                  // text region of stream 0: [0, V_text)
     int n_bridge;
     int32_t bridge[16];          // bridging tokens of the transition phase
@@ -187,6 +198,17 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
     const bool audio = cp.phase == kPhaseAudio;
     p.tokens_out[static_cast<size_t>(r) * p.S + i] = token;
     if (pm >= 0) p.tokens_out[static_cast<size_t>(pm) * p.S + i] = token;
+    if (p.xchg_tokens) {
+        // all-gather by peer stores: cell [row][GLOBAL stream] of every rank's gather buffer
+        const int gs = global_stream(p, i);
+        const size_t half = ((__ldcg(p.xchg_state + 1) + 1u) & 1u) * static_cast<size_t>(p.xchg_half_elems);
+        for (int q = 0; q < p.xchg_world; ++q) {
+            int32_t* dst = p.xchg_tokens[q] + half;
+            dst[static_cast<size_t>(r) * p.S_total + gs] = token;
+            if (pm >= 0) dst[static_cast<size_t>(pm) * p.S_total + gs] = token;
+        }
+        __threadfence_system();        // ordered before this CTA's arrival below
+    }
     if (p.delayed && audio) {          // only audio-phase tokens belong to the codebook matrix
         const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
         p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
@@ -259,6 +281,56 @@ __device__ __forceinline__ BestSV block_argmax(BestSV b, float* red_s, int* red_
     return b;
 }
 
+// Stream-sharded token exchange, end of the finalize grid (every thread of every CTA calls it): once all CTAs
+// have stored their tokens into the peers' gather buffers, the last CTA publishes this rank's next epoch in
+// flags[q][rank] of every rank q.  A rank's consumers wait until all `world` flags reached their own epoch
+// (cfgms_exchange_wait_kernel).  The epoch lives on the device, so a captured graph replays correctly.
+__device__ __forceinline__ void xchg_finish(const FinalizeParams& p) {
+    if (!p.xchg_tokens) return;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        const unsigned int total = gridDim.x * gridDim.y * gridDim.z;
+        if (atomicAdd(p.xchg_state, 1u) == total - 1u) {
+            p.xchg_state[0] = 0u;
+            const unsigned int epoch = p.xchg_state[1] + 1u;
+            p.xchg_state[1] = epoch;
+            __threadfence_system();
+            for (int q = 0; q < p.xchg_world; ++q) {
+                volatile uint32_t* f = p.xchg_flags[q] + p.xchg_rank;
+                *f = epoch;
+            }
+        }
+    }
+}
+
+// Waits (bounded) until every rank's tokens of the current step have landed in THIS rank's gather buffer —
+// flags[q] >= this rank's own wait count — and then copies the step's half into `latest`, the buffer consumers
+// read (so nothing outside this kernel needs to know the epoch: CUDA-graph replay stays correct).  One CTA.
+__global__ void __launch_bounds__(256)
+cfgms_exchange_wait_kernel(const volatile uint32_t* flags, unsigned int* wait_count, int world, const int32_t* halves,
+                           int32_t* latest, int half_elems, int n_copy, int* err) {
+    __shared__ unsigned int want;
+    if (threadIdx.x == 0) { want = *wait_count + 1u; }
+    __syncthreads();
+    if (static_cast<int>(threadIdx.x) < world) {
+        const uint64_t t0 = global_timer_ns();
+        while (static_cast<int>(flags[threadIdx.x] - want) < 0) {
+            __nanosleep(200);
+            if (global_timer_ns() - t0 > 2000000000ull) {
+                atomicCAS(err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (11 << 8));
+                __threadfence_system();
+                __trap();
+            }
+        }
+    }
+    __threadfence_system();      // acquire side
+    __syncthreads();
+    const int32_t* src = halves + static_cast<size_t>(want & 1u) * half_elems;
+    for (int e = threadIdx.x; e < n_copy; e += blockDim.x) latest[e] = __ldcv(src + e);
+    if (threadIdx.x == 0) *wait_count = want;
+}
+
 // Exact k-th largest (1-based, with multiplicity) of n keys in shared memory, by ONE warp:
 // MSB-first radix select, 8 bits per pass.  Requires 1 <= k <= n.
 struct SmemKeys {
@@ -328,7 +400,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
     const int lane = tid & 31;
     const int warp = tid >> 5;
     const int pm = p.pair_map[r];
-    if (pm >= 0 && (r & 1)) return;  // companion row: its cond row writes both
+    if (pm >= 0 && (r & 1)) { xchg_finish(p); return; }  // companion row: its cond row writes both
 
     const int gi = global_stream(p, i);
     const CellPlan cp = plan_cell(p, r, gi, __ldcg(p.step + r), p.n_frames ? __ldcg(p.n_frames + r) : 2147483647);
@@ -446,6 +518,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
         token = best.v;
     }
     if (tid == 0) write_cell(p, r, i, pm, cp, token, modality);
+    xchg_finish(p);
 }
 
 // Fallback for V > 256 * 32: keys in shared memory, radix select over all of them.
@@ -459,7 +532,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
     pdl_launch_dependents();
     const int i = blockIdx.x, r = blockIdx.y, tid = threadIdx.x;
     const int pm = p.pair_map[r];
-    if (pm >= 0 && (r & 1)) return;
+    if (pm >= 0 && (r & 1)) { xchg_finish(p); return; }
     const int gi = global_stream(p, i);
     const CellPlan cp = plan_cell(p, r, gi, __ldcg(p.step + r), p.n_frames ? __ldcg(p.n_frames + r) : 2147483647);
     const int tau = cp.gstep;          // keys the noise
@@ -509,6 +582,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
         token = best.v;
     }
     if (tid == 0) write_cell(p, r, i, pm, cp, token, modality);
+    xchg_finish(p);
 }
 
 
@@ -873,6 +947,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         CFGMS_K2_MARK(7);          // noise drawn, argmax done
     }
     if (valid && lane == 0) write_cell(p, r, i, pm, cp, token, modality);
+    xchg_finish(p);
     CFGMS_K2_MARK(8);
     if (p.ready) {
         // the last CTA to finish re-arms the counters for the next step's K1 (which starts after this grid)

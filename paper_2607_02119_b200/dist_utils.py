@@ -105,3 +105,30 @@ def all_gather_stream_tokens(tokens_local: torch.Tensor, S: int) -> torch.Tensor
     parts = [torch.empty_like(mine) for _ in range(world)]
     dist.all_gather(parts, mine)
     return merge_stream_shards(parts, S)
+
+
+# ---------------------------------------------------------------- device-side token exchange (cfgms_exchange_*)
+# The all-gather above is the CPU-testable reference of the exchange; on GPUs the finalize kernel does it itself
+# with peer stores into every rank's gather buffer + one flag per destination.  torch.distributed only carries
+# the 64-byte CUDA IPC handles at set-up time; no collective runs on the data path.
+
+def exchange_handles(handle: bytes) -> list:
+    """Every rank's exchange handle, in rank order (set-up time, any backend)."""
+    if len(handle) != 64:
+        raise ValueError("a CUDA IPC handle is 64 bytes")
+    if not dist.is_initialized():
+        return [bytes(handle)]
+    out = [None] * dist.get_world_size()
+    dist.all_gather_object(out, bytes(handle))
+    if any(h is None or len(h) != 64 for h in out):
+        raise RuntimeError("exchange handle missing from a rank")
+    return out
+
+
+def connect_stream_exchange(ctx, rank: int, world: int) -> None:
+    """Create this rank's exchange block and connect it to every peer's (one process per GPU)."""
+    handle, base = ctx.exchange_create(world, rank)
+    if world == 1:
+        ctx.exchange_connect([base])
+    else:
+        ctx.exchange_connect_ipc(exchange_handles(handle))

@@ -72,3 +72,67 @@ def test_single_process_is_identity():
         assert dist_utils.max_over_ranks(3.5) == 3.5
         rate, worst = dist_utils.whole_job_rate(1000.0, 10.0)
         assert worst == 10.0 and abs(rate - 1e5) < 1e-9
+
+
+def _exchange_worker(rank, world, port, out):
+    """Host logic of the device-side token exchange plus a CPU model of its flag protocol: each rank scatters its
+    stream columns of step e into half e & 1 of EVERY rank's gather buffer, then raises flags[q][rank] = e; a rank
+    consumes step e once all its flags reached e.  A rank can only start step e + 1 after consuming step e (its
+    next input needs everyone's tokens), which is what makes two halves enough — the model checks exactly that
+    with skewed ranks over many steps."""
+    sys.path.insert(0, ROOT)
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import time
+    from paper_2607_02119_b200 import dist_utils
+    dist_utils.init("gloo")
+    # 1. set-up: 64-byte handles gathered in rank order
+    mine = bytes([rank]) * 64
+    handles = dist_utils.exchange_handles(mine)
+    assert handles == [bytes([q]) * 64 for q in range(world)]
+    try:
+        dist_utils.exchange_handles(b"short")
+        raise AssertionError("a malformed handle must be refused")
+    except ValueError:
+        pass
+    # 2. the protocol, on shared host memory standing in for the peer-mapped blocks
+    bufs, flags = out["bufs"], out["flags"]          # [world][2][R][S] tokens, [world][world] epochs
+    S, R = bufs.shape[3], bufs.shape[2]
+    base, stride, _ = dist_utils.stream_shard(rank, world, S)
+    tok = lambda e, r, s: e * 1000 + r * 16 + s
+    ok = True
+    for e in range(1, 41):
+        if (e * 7 + rank * 3) % 5 == 0:
+            time.sleep(0.002)                        # skew the ranks
+        for q in range(world):                       # scatter: peer stores
+            for s_ in range(base, S, stride):
+                for r in range(R):
+                    bufs[q, e & 1, r, s_] = tok(e, r, s_)
+        for q in range(world):                       # publish (after the stores)
+            flags[q, rank] = e
+        t0 = time.time()
+        while int(flags[rank].min()) < e:            # wait: every rank's step e has landed here
+            assert time.time() - t0 < 20
+        got = bufs[rank, e & 1].clone()
+        want = torch.tensor([[tok(e, r, s_) for s_ in range(S)] for r in range(R)], dtype=got.dtype)
+        ok = ok and bool(torch.equal(got, want))
+        dist_utils.barrier()                         # stands in for "the next step needs everyone's tokens"
+    out[rank] = ok
+    dist.destroy_process_group()
+
+
+def _exchange_worker_entry(rank, world, port, out, bufs, flags):
+    box = {"bufs": bufs, "flags": flags}
+    _exchange_worker(rank, world, port, box)
+    out[rank] = box[rank]
+
+
+def test_two_rank_exchange_handles_and_flag_protocol():
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    # tensors in shared memory travel to the spawned ranks as handles; results come back through the manager
+    bufs = torch.zeros((world, 2, 3, 5), dtype=torch.int32).share_memory_()
+    flags = torch.zeros((world, world), dtype=torch.int64).share_memory_()
+    mp.spawn(_exchange_worker_entry, args=(world, 29617, out, bufs, flags), nprocs=world, join=True)
+    assert out[0] is True and out[1] is True

@@ -321,3 +321,76 @@ def test_ragged_stream_vocabularies_equal_truncated_heads(dev):
                 if not ref.flags[j] & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
                     assert got[c, i] == ref.tok[j], (t, c, i, Vi)
     del keep
+
+
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_device_side_token_exchange_between_stream_shards(dev, world):
+    """W5 with the exchange done by the finalize kernel itself (cfgms_exchange_*): every 'rank' — here contexts of
+    ONE process on ONE GPU, connected through their same-process block addresses, launched one after the other on
+    one stream so that no kernel ever waits for a later one — stores its tokens into every rank's gather buffer and
+    raises its flags; after the waits every rank holds the full [R][S] token matrix of the unsharded head.  Several
+    steps (epochs, both halves of the double buffer), then a CUDA-graph replay of two more."""
+    import paper_2607_02119_b200 as pkg
+    from paper_2607_02119_b200 import dist_utils
+    wl = _custom(pairs=5, singles=2, d=256, S=9, V=256, T=24, mixed=True)
+    full = DeviceWorkload(wl, dev)
+    R, S = wl.R, wl.S
+    ranks = []
+    for g in range(world):
+        base, stride, s_local = dist_utils.stream_shard(g, world, S)
+        heads = wl.heads[base::stride].contiguous().to(dev)
+        embeds = wl.embeds[base::stride].contiguous().to(dev)
+        ctx = pkg.Context(heads, embeds, max_rows=R, stream_base=base, stream_stride=stride, global_streams=S)
+        handle, addr = ctx.exchange_create(world, g)
+        assert len(handle) == 64 and addr
+        ranks.append(dict(ctx=ctx, heads=heads, embeds=embeds, addr=addr,
+                          tok=torch.full((R, s_local), -1, dtype=torch.int32, device=dev)))
+    for rk in ranks:
+        rk["ctx"].exchange_connect([x["addr"] for x in ranks])
+        rk["all"] = rk["ctx"].exchange_tokens(R, S)
+
+    def step_all(t, st):
+        for rk in ranks:
+            rk["ctx"].step(full.hidden(t), full.pair_map, full.w, full.temp, full.top_k, wl.seed, st, rk["tok"],
+                           req_id=full.req_id, n_frames=full.n_frames)
+        for rk in ranks:
+            rk["ctx"].exchange_wait(R)
+
+    for t in (0, 1, 4, 8, 9, 15, 23):
+        full.step(t)
+        step_all(t, wl.step(t).to(dev))
+        torch.cuda.synchronize()
+        for g, rk in enumerate(ranks):
+            assert torch.equal(rk["all"], full.tokens), (t, g)
+            rc, row = rk["ctx"].last_device_error()
+            assert rc == 0
+    # graph replay: the epochs live on the device
+    sts = {t: wl.step(t).to(dev) for t in (10, 11)}
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        step_all(10, sts[10])
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g, stream=s):
+        step_all(10, sts[10])
+        step_all(11, sts[11])
+    full.step(11)
+    for _ in range(3):
+        for rk in ranks:
+            rk["all"].fill_(-5)
+        g.replay()
+        torch.cuda.synchronize()
+        for rk in ranks:
+            assert torch.equal(rk["all"], full.tokens)
+    # the exchange needs the global stream count, and there is one per context
+    with pytest.raises(pkg.CfgmsError):
+        ranks[0]["ctx"].exchange_create(world, 0)
+    if world > 1:
+        lone = pkg.Context(ranks[1]["heads"], ranks[1]["embeds"], max_rows=R, stream_base=1, stream_stride=world)
+        with pytest.raises(pkg.CfgmsError):
+            lone.exchange_create(world, 1)
+        lone.close()
+    for rk in ranks:
+        rk["ctx"].close()
