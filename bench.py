@@ -26,9 +26,21 @@ if ROOT not in sys.path:
 
 METRIC = "cfg_audio_frames_per_sec"
 UNIT = "frames/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per head-GEMM launch from the committed
-# `ncu --set full` capture (profiles/), keyed by config; None until captured.
-NCU_TRAFFIC_BYTES = {5: 342.68e6}   # profiles/r1c_ncu_full_config5.md: dram read + written per head-GEMM launch
+
+
+def ncu_traffic_bytes(cfg: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per head-GEMM launch, from the committed `ncu --set full`
+    captures: profiles/ncu_traffic.csv (config,kernel,dram_bytes_per_launch,capture) holds the figure read off each
+    capture's raw page (the bench itself never runs under a profiler).  None when no capture exists for this config."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        for ln in f:
+            parts = ln.strip().split(",")
+            if len(parts) >= 3 and parts[0] == str(cfg) and parts[1] == "head_gemm":
+                return float(parts[2])
+    return None
 
 
 def load_peaks():
@@ -75,7 +87,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.002)
+            time.sleep(0.0002)
 
     def __enter__(self):
         if self.nv is not None:
@@ -98,14 +110,16 @@ class Runner:
     """One config resident on one GPU, stepping through the C ABI."""
 
     cta_pair = None   # tuning override (--cta-pair): None = library default
+    probe = 0         # measurement probes (--probes): CFGMS_CFG_PROBE_* bits for the contexts built next
 
-    def __init__(self, cfg: int, dev, cfg_off: bool = False, rank: int = 0, n_ranks: int = 1, shard_streams: bool = False):
+    def __init__(self, cfg: int, dev, cfg_off: bool = False, rank: int = 0, n_ranks: int = 1, shard_streams: bool = False,
+                 overrides=None):
         import torch
         import paper_2607_02119_b200 as pkg
         from paper_2607_02119_b200 import dist_utils
         import workloads
         self.torch = torch
-        wl = workloads.make_config(cfg, cfg_off=cfg_off)
+        wl = workloads.make_config(cfg, cfg_off=cfg_off, overrides=overrides)
         self.shard_streams = shard_streams
         self.S_local = wl.S
         self.wl, self.dev = wl, dev
@@ -125,7 +139,7 @@ class Runner:
             first, _ = dist_utils.shard_request_ids(rank, n_ranks, wl.n_req)
             wl.req_id = wl.req_id + first
             self.heads, self.embeds = cu(wl.heads), cu(wl.embeds)
-            self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), cta_pair=Runner.cta_pair)
+            self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), cta_pair=Runner.cta_pair, probe=Runner.probe)
         self.pool = cu(wl.hidden_pool)
         self.pair_map, self.w, self.temp, self.top_k = cu(wl.pair_map), cu(wl.w), cu(wl.temp), cu(wl.top_k)
         self.req_id, self.n_frames = cu(wl.req_id), cu(wl.n_frames)
@@ -175,14 +189,14 @@ class Runner:
         for t in range(warmup):
             self.step(t)
         g = self.capture(warmup, K, with_deint)
+        if sampler:      # sampled over an untimed replay of the same graph and the timed one (a 20-step replay lasts ~4 ms)
+            sampler.__enter__()
         g.replay()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         if barrier:
             barrier()
         torch.cuda.synchronize()
-        if sampler:
-            sampler.__enter__()
         e0.record()
         g.replay()
         e1.record()
@@ -326,6 +340,20 @@ class Runner:
         inf = self.ctx.info()
         return dt, inf["h2d_bytes_last_step"], inf["d2h_bytes_last_step"]
 
+    def pcie_h2d_gbs(self, mib: int = 64):
+        """What this box's host link delivers for one large pinned host->device copy (context for `e2e`)."""
+        torch = self.torch
+        src = torch.empty(mib * 2 ** 20, dtype=torch.uint8).pin_memory()
+        dst = torch.empty(mib * 2 ** 20, dtype=torch.uint8, device=self.dev)
+        dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        dst.copy_(src, non_blocking=True)
+        e1.record()
+        torch.cuda.synchronize()
+        return mib * 2 ** 20 / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
 
 def oracle_sample(wl, budget_s: float = 12.0):
     """Times the fp64 oracle, as it stands, on a bounded seeded sample of cells of one step."""
@@ -374,8 +402,11 @@ def run_reference(args):
     t0 = time.perf_counter()
     run(wl.S, cells[:n0])
     rate = n0 / (time.perf_counter() - t0)                     # cells per second
-    per_step = 100.0 / max(args.steps + args.warmup, 1)
+    per_step = 170.0 / max(args.steps + args.warmup, 1)       # the whole run ends within about three minutes
     n = int(min(len(cells), max(threads, rate * per_step)))
+    if n >= 0.8 * len(cells):
+        n = len(cells)                                           # close enough: run whole steps, nothing is extrapolated
+    full = n == len(cells)
     frames = secs = 0.0
     for j in range(args.warmup + args.steps):
         t = wl.S + (j % (wl.T - 2 * wl.S))                       # every stream active
@@ -390,9 +421,12 @@ def run_reference(args):
     cb = dict(value=value, unit=UNIT, cores=threads, kind="oracle",
               sample=f"{n} of {len(cells)} (request, stream) cells per step of {wl.name}, {args.steps} steps, {secs:.1f} s")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wl.n_req / value, "higher_is_better": True,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wl.n_req / value,
+            "ms_per_step_is": "measured: every step ran all of its cells" if full else
+                              f"extrapolated: each step ran {n} of its {len(cells)} cells, scaled to a whole step",
+            "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(wl, args.config, "cpu oracle on a bounded sample of cells per step"),
+            "config": workload_config(wl, args.config, "cpu oracle, whole steps" if full else "cpu oracle on a bounded sample of cells per step"),
             "cpu_baseline": cb,
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -418,6 +452,11 @@ def main():
                     help="multi-GPU sharding: 'requests' = independent replicas (default, weak scaling); 'streams' = every rank "
                          "holds the head slices of streams {rank, rank + N, ...}, all ranks see all rows, tokens are exchanged "
                          "by the finalize kernel through peer-mapped memory (strong scaling of the weight stream; default config 3)")
+    ap.add_argument("--quick", action="store_true",
+                    help="profiling aid: time the main graph and the kernels only (no e2e, no cpu baseline, no regimes); "
+                         "the line then lacks those keys and is not a bench record")
+    ap.add_argument("--probes", action="store_true",
+                    help="also time the two measurement probes (noise drawn in the GEMM epilogue; no logit spill) at configs 2, 3, 5")
     ap.add_argument("--cta-pair", default="auto", choices=["auto", "on", "off"],
                     help="tuning: force the CTA-pair (cta_group::2) or the one-CTA head GEMM")
     args = ap.parse_args()
@@ -467,7 +506,7 @@ def main():
             roof = {"bound": "hbm", "achieved": main_r.bytes_per_step / (gemm_us * 1e-6) / 1e9,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s"}
         roof["frac"] = roof["achieved"] / roof["peak"]
-        roof["traffic"] = NCU_TRAFFIC_BYTES.get(args.config)
+        roof["traffic"] = ncu_traffic_bytes(args.config)
         roof.update(kernel="cfgms_head_gemm_kernel", kernel_us=gemm_us, finalize_us=fin_us, peak_source=peaks["source"],
                     roofline_us_per_step=1e6 * max(t_tensor, t_hbm), step_frac=max(t_tensor, t_hbm) * 1e6 / us_per_step,
                     frac_of_sustained_peak=(roof["achieved"] / peaks["tflops_sustained"]) if roof["bound"] == "tensor" else None)
@@ -487,6 +526,13 @@ def main():
                 "clocks": sampler.summary(), "gpu_launches": int((info["launches_last_step"] + (1 if sharded else 0)) * K + (0 if sharded else 1)),
                 "roofline": roof}
 
+    if args.quick:
+        if rank == 0:
+            print(json.dumps(line))
+        if world > 1:
+            dist_utils.barrier(dev)
+            torch.distributed.destroy_process_group()
+        return
     # end-to-end through the host-buffer entry point (every rank, max over ranks)
     Ke = min(K, 64)
     dt_e2e, h2d, d2h = main_r.time_e2e(Ke, 3)
@@ -495,9 +541,28 @@ def main():
     else:
         e2e_value, _ = dist_utils.whole_job_rate(float(wl.n_req) * Ke, dt_e2e * 1e3, dev)
     if rank == 0:
+        link = main_r.pcie_h2d_gbs()
         line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                       "us_per_step": 1e6 * dt_e2e / Ke, "api": "cfgms_step_host (pinned host buffers, sync per step)"}
+                       "us_per_step": 1e6 * dt_e2e / Ke,
+                       "api": "cfgms_step_host (pinned host buffers; hidden states uploaded row block by row block on a second "
+                              "stream while the GEMM of the previous block runs; sync per step)",
+                       "host_link_h2d_gbs": link, "h2d_us_at_link_rate": h2d / link / 1e3}
 
+    if rank == 0 and world == 1 and not sharded:
+        # Both clock regimes in one line, so that the headline does not depend on --steps: a short burst (the part
+        # below its power cap) and a sustained run (>= 400 back-to-back steps: config 5 then sits at the 1 kW cap).
+        t_roof_us = line["roofline"]["roofline_us_per_step"]
+        t_roof_sus = (main_r.flops_per_step / (peaks["tflops_sustained"] * 1e12) * 1e6) if line["roofline"]["bound"] == "tensor" else t_roof_us
+        regimes = {}
+        for name, steps in (("burst", 20), ("sustained", 400)):
+            smp = ClockSampler(local_rank)
+            ms = main_r.time_graph(min(steps, wl.T), 3, with_deint=False, sampler=smp)
+            us = 1e3 * ms / min(steps, wl.T)
+            regimes[name] = {"steps": min(steps, wl.T), "us_per_step": us, "frames_per_s": wl.n_req / us * 1e6,
+                             "step_frac_of_burst_peak_roofline": t_roof_us / us,
+                             "step_frac_of_sustained_peak_roofline": t_roof_sus / us, "clocks": smp.summary()}
+        line["regimes"] = regimes
+        main_hot_us = regimes["sustained"]["us_per_step"] if K >= 100 else regimes["burst"]["us_per_step"]
     if rank == 0 and world == 1:
         cb, _, _ = oracle_sample(wl)
         line["cpu_baseline"] = cb
@@ -536,8 +601,45 @@ def main():
                 del r
                 torch.cuda.empty_cache()
             line["other_configs"] = extras
+            # the paper-style ratio (reading C22: equal ROWS, as in PAPER.md:107,163 — B pairs against 2B unpaired requests)
+            if "config2" in ratio:
+                re_ = Runner(2, dev, overrides=dict(pairs=0, singles=128))
+                ms_e = re_.time_graph(min(K, re_.wl.T), W, with_deint=False)
+                us_e = 1e3 * ms_e / min(K, re_.wl.T)
+                ratio["config2"].update(noncfg_equal_rows_us=us_e,
+                                        ratio_equal_rows_hot=(64 / ratio["config2"]["cfg_us"]) / (128 / us_e))
+                del re_
+                torch.cuda.empty_cache()
+            # config 5: both runs are tensor-bound, so the best possible ratio is t_tensor(512 rows) / t_tensor(1024 rows) = 0.5
+            if args.config == 5:
+                ro = Runner(5, dev, cfg_off=True)
+                n5 = min(K, 100)
+                hot_o = 1e3 * ro.time_graph(n5, W, with_deint=False) / n5
+                ratio["config5"] = {"cfg_us": main_hot_us, "noncfg_us": hot_o, "ratio_equal_requests_hot": hot_o / main_hot_us,
+                                    "ceiling": 0.5, "ceiling_arithmetic": "both tensor-bound: 2*512*S*d*V / (2*1024*S*d*V) = 0.50 "
+                                                                          "(84.1 us / 168.1 us at the measured burst peak)"}
+                del ro
+                torch.cuda.empty_cache()
             line["ratio"] = dict(ratio, paper_context="paper: CFG sustains 80% of non-CFG decode tok/s, whole engine, "
                                                       "1x H100 80GB, equal rows (PAPER.md:154-163)")
+        if args.probes and not sharded:
+            # The two design choices DESIGN.md section 7 argues, measured: noise drawn for every logit in the GEMM epilogue
+            # (lower bound of the fused variant: the draws are discarded) and the step without the fp32 logit spill.
+            probes = {}
+            for cfg in (2, 3, 5):
+                row = {}
+                for name, bits in (("default", 0), ("epilogue_noise", 256), ("no_spill", 512)):
+                    Runner.probe = bits
+                    r = Runner(cfg, dev)
+                    n = min(100, r.wl.T)
+                    row[name + "_us"] = 1e3 * r.time_graph(n, 5, with_deint=False) / n
+                    g_us, f_us = r.time_kernels(32, 3)
+                    row[name + "_gemm_us"] = g_us
+                    del r
+                    torch.cuda.empty_cache()
+                Runner.probe = 0
+                probes[f"config{cfg}"] = row
+            line["probes"] = probes
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -70,6 +70,13 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
                                     the GEMM runs, it fetches its per-request parameters and waits on the device
                                     (griddepcontrol.wait) for the GEMM's results                          */
 
+/* Measurement probes behind DESIGN.md section 7's two argued design choices; never part of a product run. */
+#define CFGMS_CFG_PROBE_EPILOGUE_NOISE 256u /* the head GEMM's epilogue additionally draws the Philox-Gumbel noise of
+                                    EVERY merged logit (the literal "noise fused into the epilogue"); the draws are
+                                    discarded, tokens are unchanged: a lower bound of that variant's cost           */
+#define CFGMS_CFG_PROBE_NO_SPILL 512u /* the head GEMM does not write the fp32 logit spill (timing only: cells whose
+                                    sampling needs a spilled row are then wrong)                                 */
+
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
     int32_t pad_token; /* written at inactive (step, stream) cells when CFGMS_CFG_PAD_TOKEN      */
@@ -225,6 +232,15 @@ int cfgms_set_logit_bias(cfgms_ctx* ctx, const float* bias, void* cuda_stream);
  * transition phase (copied).  Takes effect for steps enqueued afterwards.  Errors: ARG, SHAPE.
  */
 int cfgms_set_phase_table(cfgms_ctx* ctx, int32_t V_text, const int32_t* bridge_tokens, int32_t n_bridge);
+
+/*
+ * cfgms_set_stream_vocab_sizes — ragged per-stream vocabularies on the uniform [S][V][d] layout (PAPER.md:104-105:
+ * OpusLM's SSL stream and codec streams differ in size): stream i only ever samples tokens < sizes[i].
+ * sizes: HOST int32 [S], 1 <= sizes[i] <= V; extra_bias: DEVICE fp32 [S][V] additive bias applied as well, or
+ * NULL.  Replaces whatever cfgms_set_logit_bias installed (same mechanism: folded once into the per-token bias
+ * of the GEMM epilogue, -inf on the padded tail).  Errors: ARG.
+ */
+int cfgms_set_stream_vocab_sizes(cfgms_ctx* ctx, const int32_t* sizes, const float* extra_bias, void* cuda_stream);
 
 /*
  * Stream-sharded heads: the token exchange as a device-side operation (decode is memory-bound,

@@ -20,6 +20,8 @@ CFGMS_CFG_CTA_PAIR = 8
 CFGMS_CFG_NO_OVERLAP = 16
 CFGMS_CFG_OVERLAP = 32
 CFGMS_CFG_NO_PDL_FINALIZE = 64
+CFGMS_CFG_PROBE_EPILOGUE_NOISE = 256
+CFGMS_CFG_PROBE_NO_SPILL = 512
 CFGMS_FRAMES_UNSET = 2 ** 31 - 1
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
@@ -29,7 +31,8 @@ EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cf
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
            "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats",
            "cfgms_set_logit_bias", "cfgms_feedback", "cfgms_set_phase_table", "cfgms_exchange_create",
-           "cfgms_exchange_connect", "cfgms_exchange_connect_ipc", "cfgms_exchange_wait", "cfgms_exchange_tokens"]
+           "cfgms_exchange_connect", "cfgms_exchange_connect_ipc", "cfgms_exchange_wait", "cfgms_exchange_tokens",
+           "cfgms_set_stream_vocab_sizes"]
 
 
 class CfgmsError(RuntimeError):
@@ -108,6 +111,8 @@ def _lib():
         L.cfgms_exchange_wait.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
         L.cfgms_exchange_tokens.restype = C.c_int
         L.cfgms_exchange_tokens.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.cfgms_set_stream_vocab_sizes.restype = C.c_int
+        L.cfgms_set_stream_vocab_sizes.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.c_void_p, C.c_void_p]
         L.cfgms_set_phase_table.restype = C.c_int
         L.cfgms_set_phase_table.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]
         L.cfgms_feedback.restype = C.c_int
@@ -161,7 +166,7 @@ class Context:
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
                  cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0,
                  force_overlap: bool = False, stream_base: int = 0, stream_stride: int = 0,
-                 no_pdl_finalize: bool = False, global_streams: int = 0):
+                 no_pdl_finalize: bool = False, global_streams: int = 0, probe: int = 0):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -187,6 +192,7 @@ class Context:
             cfg.flags |= CFGMS_CFG_OVERLAP
         if no_pdl_finalize:        # tuning: finalize kernel always as an ordinary stream-ordered launch
             cfg.flags |= CFGMS_CFG_NO_PDL_FINALIZE
+        cfg.flags |= int(probe) & (CFGMS_CFG_PROBE_EPILOGUE_NOISE | CFGMS_CFG_PROBE_NO_SPILL)   # measurement probes (bench.py --probes)
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):
@@ -285,22 +291,18 @@ class Context:
         if rc != 0:
             raise CfgmsError(rc, "cfgms_set_logit_bias")
 
-    def set_stream_vocab_sizes(self, sizes, extra_bias: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
-        """Ragged per-stream vocabularies (e.g. one SSL stream + eight codec streams of different sizes,
-        PAPER.md:104-105) on the uniform [S][V][d] layout: stream i only ever samples tokens < sizes[i].
-        Builds the -inf vocabulary mask for the padded tail (plus `extra_bias`, fp32 [S][V], if given) and
-        installs it with cfgms_set_logit_bias.  Marshalling only: the mask is applied by the library's
-        epilogue bias.  Returns the installed bias tensor (keep it alive until the call has run)."""
+    def set_stream_vocab_sizes(self, sizes, extra_bias: Optional[torch.Tensor] = None, stream=None) -> None:
+        """cfgms_set_stream_vocab_sizes: ragged per-stream vocabularies (e.g. one SSL stream + eight codec streams
+        of different sizes) on the uniform [S][V][d] layout: stream i only ever samples tokens
+        < sizes[i]; `extra_bias` (fp32 [S][V], cuda) is added as well.  The mask is built and folded by the library."""
         sizes = [int(x) for x in sizes]
-        if len(sizes) != self.S or any(not (1 <= x <= self.V) for x in sizes):
-            raise ValueError("sizes must hold S values in [1, V]")
-        dev = self._heads.device
-        bias = torch.zeros((self.S, self.V), dtype=torch.float32, device=dev) if extra_bias is None \
-            else extra_bias.to(device=dev, dtype=torch.float32).clone()
-        col = torch.arange(self.V, device=dev).unsqueeze(0)
-        bias.masked_fill_(col >= torch.tensor(sizes, device=dev).unsqueeze(1), float("-inf"))
-        self.set_logit_bias(bias, stream=stream)
-        return bias
+        if len(sizes) != self.S:
+            raise ValueError("sizes must hold S values")
+        _check(extra_bias, "extra_bias", torch.float32, "cuda", self.S * self.V, optional=True)
+        arr = (C.c_int32 * self.S)(*sizes)
+        rc = _lib().cfgms_set_stream_vocab_sizes(self._h, arr, _ptr(extra_bias), _stream_ptr(stream))
+        if rc != 0:
+            raise CfgmsError(rc, "cfgms_set_stream_vocab_sizes")
 
     # ---- stream-sharded heads: the token exchange (cfgms_exchange_*) ----
     def exchange_create(self, world: int, rank: int):

@@ -105,6 +105,21 @@ cfgms_bias_fold_kernel(const float* __restrict__ base, const float* __restrict__
     if (e < n) bias[e] = user ? base[e] + user[e] : base[e];
 }
 
+// Same fold with ragged per-stream vocabularies (one SSL stream + eight codec streams of
+// different sizes on the uniform [S][V][d] layout): tokens v >= sizes[i] of stream i are masked with -inf.
+struct StreamSizes {
+    int32_t v[64];
+};
+__global__ void __launch_bounds__(256)
+cfgms_bias_fold_ragged_kernel(const float* __restrict__ base, const float* __restrict__ user, float* __restrict__ bias,
+                              int n, int V, const StreamSizes sizes) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int i = e / V, v = e - i * V;
+    const float b = user ? base[e] + user[e] : base[e];
+    bias[e] = v < sizes.v[i] ? b : -INFINITY;
+}
+
 // ---------------------------------------------------------------- K7 (PAPER.md:56 feedback)
 // x[r][:] = bf16( sum_i emb[i][tokens[r][i]][:] ), fp32 accumulation in stream order.  One CTA per
 // two-row slot; every thread owns 16-byte (8 x bf16) column chunks and keeps up to kFbUnroll

@@ -29,10 +29,12 @@ constexpr int kOverlapMinWaves = 3;
 
 struct HostStage {  // device staging for the *_host entry points
     void* hidden = nullptr;
-    int32_t *pair_map = nullptr, *top_k = nullptr, *step = nullptr, *n_frames = nullptr, *tokens = nullptr;
-    float *w = nullptr, *temp = nullptr;
-    uint32_t* req_id = nullptr;
-    int32_t *force_token = nullptr, *frame = nullptr, *frame_index = nullptr;
+    char* params = nullptr;        // device: one block for every small per-row input of a step (one H2D copy)
+    char* params_pinned = nullptr; // pinned host mirror the caller's arrays are packed into
+    size_t params_bytes = 0;
+    int32_t *tokens = nullptr, *frame = nullptr, *frame_index = nullptr;
+    cudaStream_t copy_stream = nullptr;   // hidden-state row blocks are uploaded here while the GEMM of the previous block runs
+    cudaEvent_t chunk_ev[16] = {nullptr};
     int32_t* deint_in = nullptr;
     int32_t* deint_out = nullptr;
     size_t deint_in_bytes = 0, deint_out_bytes = 0;
@@ -51,6 +53,7 @@ struct cfgms_ctx {
     int poll_ns = 2000;       // K2's sleep between polls of a ready counter: 1-4 us measured ~2.4 % faster than 50-200 ns at config 5
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     bool pdl_finalize = true;         // serial mode: launch a small K2 grid as a programmatic dependent of K1
+    int probe = 0;                    // measurement probes (CFGMS_CFG_PROBE_*), see GemmParams::probe
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT] what the epilogue adds: bias_base (+ the caller's logit bias)
     float* bias_base = nullptr;       // [NT] W_i e_i, folded at create
@@ -242,6 +245,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     cudaMemset(c->err, 0, 2 * sizeof(int));
     c->overlap_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_OVERLAP)) ? 2 : 0;
     c->pdl_finalize = !(cfg && (cfg->flags & CFGMS_CFG_NO_PDL_FINALIZE));
+    c->probe = (cfg && (cfg->flags & CFGMS_CFG_PROBE_EPILOGUE_NOISE) ? 1 : 0) | (cfg && (cfg->flags & CFGMS_CFG_PROBE_NO_SPILL) ? 2 : 0);
     c->overlap = c->use_cand && (V % kBM) == 0 && c->overlap_mode != 1;
     if (c->overlap) {
         c->ready_words = ((S * ((c->max_rows + 63) / 64) + 1 + 1) & ~1) + 32;   // counters | done | pad | stats (16 x u64)
@@ -329,21 +333,33 @@ void cfgms_destroy(cfgms_ctx* c) {
         delete[] c->prof_ev;
     }
     HostStage& h = c->hs;
-    cudaFree(h.hidden); cudaFree(h.pair_map); cudaFree(h.top_k); cudaFree(h.step); cudaFree(h.n_frames);
-    cudaFree(h.tokens); cudaFree(h.w); cudaFree(h.temp); cudaFree(h.req_id);
-    cudaFree(h.force_token); cudaFree(h.frame); cudaFree(h.frame_index); cudaFree(h.deint_in); cudaFree(h.deint_out);
+    cudaFree(h.hidden); cudaFree(h.params); cudaFreeHost(h.params_pinned);
+    cudaFree(h.tokens); cudaFree(h.frame); cudaFree(h.frame_index); cudaFree(h.deint_in); cudaFree(h.deint_out);
+    for (int j = 0; j < 16; ++j)
+        if (h.chunk_ev[j]) cudaEventDestroy(h.chunk_ev[j]);
+    if (h.copy_stream) cudaStreamDestroy(h.copy_stream);
     delete c;
 }
 
-int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
-    int rc = validate_step(c, a);
-    if (rc != CFGMS_OK) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+}  // extern "C"
+
+namespace {
+
+// Host-buffer mode of a step (cfgms_step_host): the hidden states are still in (pinned) host memory; they are
+// uploaded one GEMM row block at a time on a second stream while the GEMM of the previous row block runs.
+struct HostUpload {
+    const char* host_hidden;   // bf16 [R][d] on the host
+    char* dev_hidden;          // staging on the device
+    int64_t* h2d_bytes;
+};
+
+int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const HostUpload* up) {
+    int rc = CFGMS_OK;
     int launches = 0;
 
     // K5: fp32 hidden -> bf16 (RNE)
-    const __nv_bfloat16* hidden = static_cast<const __nv_bfloat16*>(a->hidden);
-    if (a->hidden_dtype == CFGMS_F32) {
+    const __nv_bfloat16* hidden = up ? reinterpret_cast<const __nv_bfloat16*>(up->dev_hidden) : static_cast<const __nv_bfloat16*>(a->hidden);
+    if (!up && a->hidden_dtype == CFGMS_F32) {
         const size_t n = static_cast<size_t>(a->R) * c->d;
         if ((reinterpret_cast<uintptr_t>(a->hidden) & 15u) != 0) return CFGMS_ERR_ARG;
         const int blocks = static_cast<int>(std::min<size_t>((n / 4 + 255) / 256 + 1, static_cast<size_t>(c->num_sms) * 8));
@@ -357,7 +373,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     bool pair;
     choose_row_tile(c, a->R, &BN, &nrb, &pair);
     const int b_rows = pair ? BN / 2 : BN;     // batch rows one CTA stages per K block (TMA box height)
-    if (c->tmap_h_ptr != hidden || c->tmap_h_R != a->R || c->tmap_h_box != b_rows) {
+    if (!up && (c->tmap_h_ptr != hidden || c->tmap_h_R != a->R || c->tmap_h_box != b_rows)) {
         rc = make_tmap_2d(c, &c->tmap_h, hidden, static_cast<uint64_t>(a->R), static_cast<uint64_t>(c->d),
                           static_cast<uint32_t>(b_rows));
         if (rc != CFGMS_OK) return rc;
@@ -384,9 +400,10 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     // the polling finalize warps then cost more than the early launch saves (measured).
     // (While the profiling events are recorded the SAME kernels run, but K2 is launched strictly after K1 so
     // that each has a duration of its own.)
-    const bool overlap = c->overlap && (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
+    const bool overlap = !up && c->overlap && (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
     gp.ready = overlap ? c->ready : nullptr;
     gp.V = c->V;
+    gp.probe = c->probe; gp.probe_sink = reinterpret_cast<uint32_t*>(c->err + 1);
     gp.split_tma = gp.num_tiles < kOverlapMinWaves * workers ? 1 : 0;
     // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
     gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
@@ -396,8 +413,33 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     gp.trace = c->trace_k1;
 #endif
     const size_t smem = GemmSmemLayout::total(b_rows, stages);
+    gp.row0 = 0;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
-    {
+    // One launch for the whole batch — or, in host-buffer mode, one launch per uploaded row block: block k + 1 crosses
+    // PCIe while the GEMM of block k runs (each launch re-streams the weights, which the tensor-bound regime hides).
+    const int n_launch = up ? nrb : 1;
+    if (n_launch > 15) return CFGMS_ERR_SHAPE;      // chunk events 0..14 (15 orders the copy stream behind the caller's)
+    for (int k = 0; k < n_launch; ++k) {
+        CUtensorMap tmap_chunk;
+        const CUtensorMap* tmap_h = &c->tmap_h;
+        if (up) {
+            HostStage& hs = c->hs;
+            const int row0 = k * BN, rows = std::min(BN, a->R - row0);
+            const size_t off = static_cast<size_t>(row0) * c->d * 2, bytes = static_cast<size_t>(rows) * c->d * 2;
+            if (cudaMemcpyAsync(up->dev_hidden + off, up->host_hidden + off, bytes, cudaMemcpyHostToDevice, hs.copy_stream) != cudaSuccess ||
+                cudaEventRecord(hs.chunk_ev[k], hs.copy_stream) != cudaSuccess ||
+                cudaStreamWaitEvent(st, hs.chunk_ev[k], 0) != cudaSuccess)
+                return CFGMS_ERR_CUDA;
+            *up->h2d_bytes += static_cast<int64_t>(bytes);
+            rc = make_tmap_2d(c, &tmap_chunk, up->dev_hidden + off, static_cast<uint64_t>(rows), static_cast<uint64_t>(c->d),
+                              static_cast<uint32_t>(b_rows));
+            if (rc != CFGMS_OK) return rc;
+            tmap_h = &tmap_chunk;
+            gp.row0 = row0; gp.R = rows; gp.num_row_blocks = 1;
+            gp.num_tiles = pair ? (gp.num_vocab_tiles + 1) / 2 : gp.num_vocab_tiles;
+        }
+        const int launch_workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
+        const int launch_grid = pair ? 2 * launch_workers : launch_workers;
         using KernelFn = void (*)(const CUtensorMap, const CUtensorMap, const GemmParams);
         static const KernelFn table[8] = {
             cfgms_head_gemm_kernel<false, false, false>, cfgms_head_gemm_kernel<true, false, false>,
@@ -409,7 +451,7 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         const KernelFn fn = overlap ? lean[(a->logits_out ? 1 : 0) | (pair ? 2 : 0)]
                                     : table[(a->logits_out ? 1 : 0) | (c->use_cand ? 2 : 0) | (pair ? 4 : 0)];
         cudaLaunchConfig_t lc{};
-        lc.gridDim = dim3(static_cast<unsigned>(grid));
+        lc.gridDim = dim3(static_cast<unsigned>(launch_grid));
         lc.blockDim = dim3(kGemmThreads);
         lc.dynamicSmemBytes = smem;
         lc.stream = st;
@@ -424,9 +466,9 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
         attr[1].val.programmaticStreamSerializationAllowed = 1;
         lc.attrs = attr;
         lc.numAttrs = (c->overlap_mode == 1 || prof) ? 1 : 2;
-        if (cudaLaunchKernelEx(&lc, fn, c->tmap_w, c->tmap_h, gp) != cudaSuccess) return CFGMS_ERR_CUDA;
+        if (cudaLaunchKernelEx(&lc, fn, c->tmap_w, *tmap_h, gp) != cudaSuccess) return CFGMS_ERR_CUDA;
+        ++launches;
     }
-    ++launches;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 1], st);
 
     FinalizeParams fp;
@@ -524,42 +566,82 @@ int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     return CFGMS_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+int cfgms_step(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
+    const int rc = validate_step(c, a);
+    if (rc != CFGMS_OK) return rc;
+    return step_impl(c, a, static_cast<cudaStream_t>(cuda_stream), nullptr);
+}
+
 int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     int rc = validate_step(c, a);
     if (rc != CFGMS_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     HostStage& h = c->hs;
+    const size_t Rmax = static_cast<size_t>(c->max_rows);
     if (!c->hs_ready) {
-        const size_t R = static_cast<size_t>(c->max_rows);
-        if (cudaMalloc(&h.hidden, R * c->d * 4) != cudaSuccess) return CFGMS_ERR_NOMEM;
-        if (dev_alloc(&h.pair_map, R) || dev_alloc(&h.top_k, R) || dev_alloc(&h.step, R) || dev_alloc(&h.n_frames, R) ||
-            dev_alloc(&h.tokens, R * c->S) || dev_alloc(&h.w, R) || dev_alloc(&h.temp, R) || dev_alloc(&h.req_id, R) ||
-            dev_alloc(&h.force_token, R * c->S) || dev_alloc(&h.frame, R * c->S) || dev_alloc(&h.frame_index, R))
+        // every per-row input of a step travels in ONE block: seven [R] arrays + force_token [R][S]
+        h.params_bytes = Rmax * 4 * (7 + static_cast<size_t>(c->S));
+        bool ok = cudaMalloc(&h.hidden, Rmax * c->d * 4) == cudaSuccess &&
+                  cudaMalloc(reinterpret_cast<void**>(&h.params), h.params_bytes) == cudaSuccess &&
+                  cudaMallocHost(reinterpret_cast<void**>(&h.params_pinned), h.params_bytes) == cudaSuccess &&
+                  dev_alloc(&h.tokens, Rmax * c->S) == CFGMS_OK && dev_alloc(&h.frame, Rmax * c->S) == CFGMS_OK &&
+                  dev_alloc(&h.frame_index, Rmax) == CFGMS_OK &&
+                  cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+        for (int j = 0; ok && j < 16; ++j) ok = cudaEventCreateWithFlags(&h.chunk_ev[j], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) {      // leave nothing half-built behind: the next call starts over
+            cudaFree(h.hidden); cudaFree(h.params); cudaFreeHost(h.params_pinned);
+            cudaFree(h.tokens); cudaFree(h.frame); cudaFree(h.frame_index);
+            for (int j = 0; j < 16; ++j) { if (h.chunk_ev[j]) cudaEventDestroy(h.chunk_ev[j]); h.chunk_ev[j] = nullptr; }
+            if (h.copy_stream) cudaStreamDestroy(h.copy_stream);
+            h.hidden = nullptr; h.params = nullptr; h.params_pinned = nullptr; h.tokens = h.frame = h.frame_index = nullptr;
+            h.copy_stream = nullptr;
             return CFGMS_ERR_NOMEM;
+        }
         c->hs_ready = true;
     }
     const size_t R = static_cast<size_t>(a->R);
-    const size_t hid_bytes = R * c->d * (a->hidden_dtype == CFGMS_F32 ? 4 : 2);
     int64_t h2d = 0;
-    auto up = [&](void* dst, const void* src, size_t bytes) {
-        h2d += static_cast<int64_t>(bytes);
-        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    // pack the small arrays into the pinned mirror (a few tens of KB), one copy for all of them
+    size_t off = 0;
+    auto pack = [&](const void* src, size_t bytes) -> char* {
+        if (!src) return nullptr;
+        std::memcpy(h.params_pinned + off, src, bytes);
+        char* dev = h.params + off;
+        off += bytes;
+        return dev;
     };
-    bool ok = up(h.hidden, a->hidden, hid_bytes) && up(h.pair_map, a->pair_map, R * 4) && up(h.w, a->w, R * 4) &&
-              up(h.temp, a->temp, R * 4) && up(h.top_k, a->top_k, R * 4) && up(h.step, a->step, R * 4);
-    if (ok && a->req_id) ok = up(h.req_id, a->req_id, R * 4);
-    if (ok && a->n_frames) ok = up(h.n_frames, a->n_frames, R * 4);
-    if (ok && a->force_token) ok = up(h.force_token, a->force_token, R * c->S * 4);
-    if (!ok) return CFGMS_ERR_CUDA;
     cfgms_step_args d = *a;
-    d.hidden = h.hidden; d.pair_map = h.pair_map; d.w = h.w; d.temp = h.temp; d.top_k = h.top_k; d.step = h.step;
-    d.req_id = a->req_id ? h.req_id : nullptr;
-    d.n_frames = a->n_frames ? h.n_frames : nullptr;
+    d.pair_map = reinterpret_cast<const int32_t*>(pack(a->pair_map, R * 4));
+    d.w = reinterpret_cast<const float*>(pack(a->w, R * 4));
+    d.temp = reinterpret_cast<const float*>(pack(a->temp, R * 4));
+    d.top_k = reinterpret_cast<const int32_t*>(pack(a->top_k, R * 4));
+    d.step = reinterpret_cast<const int32_t*>(pack(a->step, R * 4));
+    d.req_id = reinterpret_cast<const uint32_t*>(pack(a->req_id, R * 4));
+    d.n_frames = reinterpret_cast<const int32_t*>(pack(a->n_frames, R * 4));
+    d.force_token = reinterpret_cast<const int32_t*>(pack(a->force_token, R * c->S * 4));
+    if (cudaMemcpyAsync(h.params, h.params_pinned, off, cudaMemcpyHostToDevice, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    h2d += static_cast<int64_t>(off);
     d.tokens_out = h.tokens;
-    d.force_token = a->force_token ? h.force_token : nullptr;
     d.frame_out = a->frame_out ? h.frame : nullptr;
     d.frame_index_out = a->frame_index_out ? h.frame_index : nullptr;
-    rc = cfgms_step(c, &d, cuda_stream);
+    d.hidden = h.hidden;
+    if (a->hidden_dtype == CFGMS_BF16) {
+        // hidden states: uploaded row block by row block on the copy stream, each block's GEMM launch waits for its own
+        // block only (step_impl).  The copy stream first waits for whatever precedes this call on the caller's stream.
+        if (cudaEventRecord(h.chunk_ev[15], st) != cudaSuccess || cudaStreamWaitEvent(h.copy_stream, h.chunk_ev[15], 0) != cudaSuccess)
+            return CFGMS_ERR_CUDA;
+        HostUpload up{static_cast<const char*>(a->hidden), static_cast<char*>(h.hidden), &h2d};
+        rc = step_impl(c, &d, st, &up);
+    } else {
+        const size_t hid_bytes = R * c->d * 4;
+        if (cudaMemcpyAsync(h.hidden, a->hidden, hid_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return CFGMS_ERR_CUDA;
+        h2d += static_cast<int64_t>(hid_bytes);
+        rc = step_impl(c, &d, st, nullptr);
+    }
     if (rc != CFGMS_OK) return rc;
     const size_t tok_bytes = R * c->S * 4;
     if (cudaMemcpyAsync(a->tokens_out, h.tokens, tok_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return CFGMS_ERR_CUDA;
@@ -582,6 +664,22 @@ int cfgms_set_logit_bias(cfgms_ctx* c, const float* bias, void* cuda_stream) {
     if (!c) return CFGMS_ERR_ARG;
     const int blocks = (c->NT + 255) / 256;
     cfgms_bias_fold_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->bias_base, bias, c->bias, c->NT);
+    if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
+    c->info.launches_total += 1;
+    return CFGMS_OK;
+}
+
+int cfgms_set_stream_vocab_sizes(cfgms_ctx* c, const int32_t* sizes, const float* extra_bias, void* cuda_stream) {
+    if (!c || !sizes) return CFGMS_ERR_ARG;
+    StreamSizes sz;
+    for (int i = 0; i < 64; ++i) sz.v[i] = 0;
+    for (int i = 0; i < c->S; ++i) {
+        if (sizes[i] < 1 || sizes[i] > c->V) return CFGMS_ERR_ARG;
+        sz.v[i] = sizes[i];
+    }
+    const int blocks = (c->NT + 255) / 256;
+    cfgms_bias_fold_ragged_kernel<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->bias_base, extra_bias, c->bias,
+                                                                                            c->NT, c->V, sz);
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.launches_total += 1;
     return CFGMS_OK;

@@ -36,6 +36,7 @@
 // the GEMM is still running.
 #pragma once
 #include "ptx_sm100.cuh"
+#include "finalize.cuh"   // gumbel_noise (the epilogue-noise measurement probe below)
 
 namespace cfgms {
 
@@ -64,6 +65,9 @@ struct __align__(16) SlotCoefB {
 
 struct GemmParams {
     int R, NT, d, BN, num_row_blocks, num_vocab_tiles, num_tiles, num_kb, stages;
+    int row0;            // batch row of this launch's first row: the host-buffer entry point launches the GEMM once per
+                         // uploaded row block (rows [row0, row0 + R) of the batch; the hidden-state tensor map covers
+                         // exactly those rows), everything else launches it once with row0 = 0
     const int32_t* pair_map;
     const float* w;
     const float* temp;
@@ -77,6 +81,13 @@ struct GemmParams {
     int* ready;          // nullable [S][num_row_blocks]: epilogue-warp arrivals per (stream, row block), see K2
     int V;               // tokens per stream (ready != nullptr requires V % kBM == 0)
     int split_tma;       // 1: warp 2 issues the row-tile loads; 0: warp 0 issues both (warp 2 idles)
+    // Measurement probes for the two design choices DESIGN.md section 7 argues (never set by default):
+    //   probe bit 0: draw the Philox-Gumbel noise of EVERY merged logit in this epilogue (north_star's literal
+    //                fusion) — the draws are folded into a sink word, results are unchanged: a lower bound of what
+    //                the fused variant costs;
+    //   probe bit 1: do not write the z spill (timing only: cells that need a spilled row sample garbage).
+    int probe;
+    uint32_t* probe_sink;
     uint64_t policy_w, policy_h;
 #ifdef CFGMS_TRACE
     unsigned long long* trace;
@@ -99,10 +110,11 @@ struct GemmSmemLayout {
 __device__ __forceinline__ void make_slot_coef(const GemmParams& p, int r0, SlotCoefA& a, SlotCoefB& b) {
     a = {0.f, 0.f, 0.f, 0};
     b = {0.f, 0.f, 0.f, 0.f};
-    const int r1 = r0 + 1;
-    if (r0 >= p.R) return;
+    const int r1 = r0 + 1;          // r0, r1: rows of the BATCH (pair_map holds batch rows)
+    const int r_end = p.row0 + p.R;
+    if (r0 >= r_end) return;
     const int pm0 = p.pair_map[r0];
-    const int pm1 = r1 < p.R ? p.pair_map[r1] : -1;
+    const int pm1 = r1 < r_end ? p.pair_map[r1] : -1;
     const float t0 = p.temp[r0];
     const float it0 = t0 == 0.f ? 1.f : 1.f / t0;
     if (pm0 == r1 && pm1 == r0) {                       // (cond, uncond) pair: Eq. 1
@@ -114,7 +126,7 @@ __device__ __forceinline__ void make_slot_coef(const GemmParams& p, int r0, Slot
     } else if (pm0 == -1 && pm1 == -1) {                // two unpaired rows
         a.c00 = it0; a.d0 = it0; a.kind = 1;
         b.m00 = 1.f;
-        if (r1 < p.R) {
+        if (r1 < r_end) {
             const float t1 = p.temp[r1];
             const float it1 = t1 == 0.f ? 1.f : 1.f / t1;
             b.c11 = it1; b.d1 = it1;
@@ -336,7 +348,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             // coefficients of every slot, once (the first mainloop hides it)
             for (int slot = et; slot < p.num_row_blocks * slots_per_rb; slot += 32 * kEpiWarps) {
                 SlotCoefA ca; SlotCoefB cb;
-                make_slot_coef(p, 2 * slot, ca, cb);
+                make_slot_coef(p, p.row0 + 2 * slot, ca, cb);
                 coef_a[slot] = ca; coef_b[slot] = cb;
             }
             named_bar_sync(1, 32 * kEpiWarps);
@@ -352,7 +364,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 named_bar_sync(1, 32 * kEpiWarps);    // everyone finished reading the old table
                 if (et < slots_per_rb) {
                     SlotCoefA ca; SlotCoefB cb;
-                    make_slot_coef(p, rb * BN + 2 * et, ca, cb);
+                    make_slot_coef(p, p.row0 + rb * BN + 2 * et, ca, cb);
                     coef_a[et] = ca; coef_b[et] = cb;
                 }
                 named_bar_sync(1, 32 * kEpiWarps);
@@ -385,7 +397,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                     __syncwarp();
                     if (lane == 0) { if (kPair && !leader) mbar_arrive_cluster(tempty_sig + 8 * acc); else mbar_arrive(bar_tempty + 8 * acc); }
                 }
-                const int row_base = rb * BN + sp * 64;
+                const int row_base = p.row0 + rb * BN + sp * 64;      // batch row of the slab pair's first column
                 const SlotCoefA* ca = coef_a + slot_base + sp * 32;
                 const SlotCoefB* cb = coef_b + slot_base + sp * 32;
                 float* zp = p.z + static_cast<size_t>(row_base) * NT + n;
@@ -407,7 +419,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                         const float z0 = fmaf(c.c00, a0, fmaf(c.c01, a1, bias * c.d0));
                         const bool own = (c.kind & own_even) != 0;
                         any_odd |= c.kind;
-                        if (own) st_global_f32(zq, z0);
+                        if (own && !(p.probe & 2)) st_global_f32(zq, z0);
                         if (kTap) {
                             if (own) { const SlotCoefB t = cb[j]; *reinterpret_cast<float*>(tq) = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
                             tq += row_stride;
@@ -415,6 +427,16 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                         zq += row_stride;
                         if (kCand) stg[j * kStgPitch + lane] = own ? z0 + 0.0f : -INFINITY;
                     }
+                }
+                if (kCand && (p.probe & 1)) {
+                    // measurement probe: the noise of every merged logit of the slab pair, drawn here (rolled loop over
+                    // the staged z values so that the product path's code stays as it is)
+                    uint32_t sink = 0u;
+#pragma unroll 1
+                    for (int j = 0; j < 32; ++j)
+                        sink ^= __float_as_uint(stg[j * kStgPitch + lane] +
+                                                gumbel_noise(0x1234u, 0x5678u, static_cast<uint32_t>(row_base + 2 * j), 7, n >> 11, n & 2047));
+                    if (sink == 0x9e3779b9u) *p.probe_sink = sink;    // keeps the draws alive
                 }
                 if (kCand) {
                     __syncwarp();

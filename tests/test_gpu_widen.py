@@ -305,7 +305,7 @@ def test_ragged_stream_vocabularies_equal_truncated_heads(dev):
     wl.top_k[:] = 30
     sizes = [512, 200, 200, 384, 64, 512, 100, 37, 256]
     dw = DeviceWorkload(wl, dev)
-    keep = dw.ctx.set_stream_vocab_sizes(sizes)
+    dw.ctx.set_stream_vocab_sizes(sizes)
     for t in (9, 12):
         dw.tokens.fill_(-1)
         dw.step(t)
@@ -320,7 +320,6 @@ def test_ragged_stream_vocabularies_equal_truncated_heads(dev):
                 assert got[c, i] < Vi
                 if not ref.flags[j] & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
                     assert got[c, i] == ref.tok[j], (t, c, i, Vi)
-    del keep
 
 
 @pytest.mark.parametrize("world", [1, 2, 3])
