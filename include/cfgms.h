@@ -70,6 +70,11 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
                                     the GEMM runs, it fetches its per-request parameters and waits on the device
                                     (griddepcontrol.wait) for the GEMM's results                          */
 
+#define CFGMS_CFG_NO_SPLIT_K 128u /* tuning/debug: never run a one-wave head GEMM as split-K clusters of four CTAs
+                                    (two CTA pairs that each stream half of K and exchange partial sums over
+                                    distributed shared memory; the default whenever the (vocabulary tile pair,
+                                    128-row block) tiles fill at most a quarter of the SMs)                   */
+
 /* Measurement probes behind DESIGN.md section 7's two argued design choices; never part of a product run. */
 #define CFGMS_CFG_PROBE_EPILOGUE_NOISE 256u /* the head GEMM's epilogue additionally draws the Philox-Gumbel noise of
                                     EVERY merged logit (the literal "noise fused into the epilogue"); the draws are
@@ -319,6 +324,8 @@ typedef struct {
     int64_t d2h_bytes_last_step;
     int32_t cta_pair;              /* 1 when the last head GEMM ran on CTA pairs (cta_group::2) */
     int32_t overlap;               /* 1 when the last finalize launch overlapped the head GEMM  */
+    int32_t split_k;               /* 2 when the last head GEMM ran as split-K clusters of four CTAs, else 1 */
+    int32_t reserved0;
 } cfgms_info;
 int cfgms_get_info(cfgms_ctx* ctx, cfgms_info* out);
 

@@ -20,6 +20,7 @@ CFGMS_CFG_CTA_PAIR = 8
 CFGMS_CFG_NO_OVERLAP = 16
 CFGMS_CFG_OVERLAP = 32
 CFGMS_CFG_NO_PDL_FINALIZE = 64
+CFGMS_CFG_NO_SPLIT_K = 128
 CFGMS_CFG_PROBE_EPILOGUE_NOISE = 256
 CFGMS_CFG_PROBE_NO_SPILL = 512
 CFGMS_FRAMES_UNSET = 2 ** 31 - 1
@@ -65,7 +66,8 @@ class cfgms_info(C.Structure):
                 ("row_blocks", C.c_int32), ("vocab_tiles", C.c_int32), ("gemm_grid", C.c_int32),
                 ("pipeline_stages", C.c_int32), ("launches_last_step", C.c_int32),
                 ("launches_total", C.c_int64), ("h2d_bytes_last_step", C.c_int64),
-                ("d2h_bytes_last_step", C.c_int64), ("cta_pair", C.c_int32), ("overlap", C.c_int32)]
+                ("d2h_bytes_last_step", C.c_int64), ("cta_pair", C.c_int32), ("overlap", C.c_int32),
+                ("split_k", C.c_int32), ("reserved0", C.c_int32)]
 
 
 _LIB = None
@@ -166,7 +168,8 @@ class Context:
                  pad_token: Optional[int] = None, row_tile: int = 0, no_candidates: bool = False,
                  cta_pair: Optional[bool] = None, no_overlap: bool = False, max_stages: int = 0,
                  force_overlap: bool = False, stream_base: int = 0, stream_stride: int = 0,
-                 no_pdl_finalize: bool = False, global_streams: int = 0, probe: int = 0):
+                 no_pdl_finalize: bool = False, global_streams: int = 0, probe: int = 0,
+                 no_split_k: bool = False):
         _check(heads, "heads", torch.bfloat16, "cuda")
         _check(embeds, "embeds", torch.bfloat16, "cuda")
         if heads.dim() != 3 or embeds.dim() != 2 or embeds.shape != (heads.shape[0], heads.shape[2]):
@@ -192,6 +195,8 @@ class Context:
             cfg.flags |= CFGMS_CFG_OVERLAP
         if no_pdl_finalize:        # tuning: finalize kernel always as an ordinary stream-ordered launch
             cfg.flags |= CFGMS_CFG_NO_PDL_FINALIZE
+        if no_split_k:             # tuning: never run a one-wave head GEMM as split-K clusters
+            cfg.flags |= CFGMS_CFG_NO_SPLIT_K
         cfg.flags |= int(probe) & (CFGMS_CFG_PROBE_EPILOGUE_NOISE | CFGMS_CFG_PROBE_NO_SPILL)   # measurement probes (bench.py --probes)
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()

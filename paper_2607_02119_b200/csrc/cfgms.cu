@@ -52,6 +52,7 @@ struct cfgms_ctx {
     int32_t bridge[16] = {0};
     int poll_ns = 2000;       // K2's sleep between polls of a ready counter: 1-4 us measured ~2.4 % faster than 50-200 ns at config 5
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
+    int split_mode = 0;               // split-K for one-wave GEMMs: 0 = chosen per step, 1 = never
     bool pdl_finalize = true;         // serial mode: launch a small K2 grid as a programmatic dependent of K1
     int probe = 0;                    // measurement probes (CFGMS_CFG_PROBE_*), see GemmParams::probe
     const __nv_bfloat16* heads = nullptr;
@@ -112,8 +113,22 @@ int make_tmap_2d(cfgms_ctx* c, CUtensorMap* m, const void* base, uint64_t rows, 
 // Batch rows per accumulator tile (BN, a multiple of 64 = one slab pair of the epilogue, <= 256 =
 // UMMA N with two accumulator stages in 512 TMEM columns) and whether two CTAs pair up on one
 // M = 256 MMA.  A (cond, uncond) pair never straddles a tile because BN is even.
-void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb, bool* pair) {
+void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb, bool* pair, bool* split) {
     const int vt = (c->NT + kBM - 1) / kBM;
+    *split = false;
+    // One-wave GEMMs (small batch x small vocabulary: the weight-streaming regime): when the (vocabulary
+    // tile pair, 128-row block) tiles fill at most half of the CTA pairs, every tile is given to a cluster of FOUR CTAs,
+    // two pairs that each stream half of K and exchange partial sums over DSMEM (head_gemm.cuh).  Against splitting
+    // the rows instead (two 64-row blocks, each re-reading the weight tile from L2) this halves the bytes an SM
+    // takes in (L2 -> SM is the wall there) and spreads the epilogue over all eight warps.
+    if (c->split_mode != 1 && c->overlap_mode != 2 && c->row_tile_override == 0 && c->pair_mode != 1 && vt >= 2 && c->d >= 8 * kBK) {
+        const int rb = (R + 127) / 128;
+        const int tiles = ((vt + 1) / 2) * rb;
+        if (rb * 64 <= kCoefSlots && tiles * 4 <= c->num_sms) {
+            *BN = 128; *nrb = rb; *pair = true; *split = true;
+            return;
+        }
+    }
     if (c->row_tile_override > 0) {
         *BN = c->row_tile_override;
         *nrb = (R + *BN - 1) / *BN;
@@ -245,6 +260,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     cudaMemset(c->err, 0, 2 * sizeof(int));
     c->overlap_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_OVERLAP)) ? 2 : 0;
     c->pdl_finalize = !(cfg && (cfg->flags & CFGMS_CFG_NO_PDL_FINALIZE));
+    c->split_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_SPLIT_K)) ? 1 : 0;
     c->probe = (cfg && (cfg->flags & CFGMS_CFG_PROBE_EPILOGUE_NOISE) ? 1 : 0) | (cfg && (cfg->flags & CFGMS_CFG_PROBE_NO_SPILL) ? 2 : 0);
     c->overlap = c->use_cand && (V % kBM) == 0 && c->overlap_mode != 1;
     if (c->overlap) {
@@ -285,6 +301,10 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, false, true>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<false, true, true>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_kernel<true, true, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_splitk_kernel<false, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_splitk_kernel<true, false>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_splitk_kernel<false, true>));
+    set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_splitk_kernel<true, true>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<false, false>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<true, false>));
     set_smem(reinterpret_cast<const void*>(cfgms_head_gemm_lean_kernel<false, true>));
@@ -370,8 +390,14 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     if ((reinterpret_cast<uintptr_t>(hidden) & 15u) != 0) return CFGMS_ERR_ARG;
 
     int BN, nrb;
-    bool pair;
-    choose_row_tile(c, a->R, &BN, &nrb, &pair);
+    bool pair, split;
+    choose_row_tile(c, a->R, &BN, &nrb, &pair, &split);
+    if (up) {            // host-buffer mode launches the GEMM per row block: the plain tiling
+        const int keep = c->split_mode;
+        c->split_mode = 1;
+        choose_row_tile(c, a->R, &BN, &nrb, &pair, &split);
+        c->split_mode = keep;
+    }
     const int b_rows = pair ? BN / 2 : BN;     // batch rows one CTA stages per K block (TMA box height)
     if (!up && (c->tmap_h_ptr != hidden || c->tmap_h_R != a->R || c->tmap_h_box != b_rows)) {
         rc = make_tmap_2d(c, &c->tmap_h, hidden, static_cast<uint64_t>(a->R), static_cast<uint64_t>(c->d),
@@ -393,22 +419,24 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp; gp.phase = a->phase;
     gp.bias = c->bias; gp.z = c->z; gp.tap = a->logits_out; gp.err = c->err;
     gp.cand_val = c->cand_val; gp.cand_src = c->cand_src;
-    const int workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
+    const int workers = split ? gp.num_tiles : std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
     const bool prof = c->prof_on && c->prof_n < kProfMax;
     // Overlap K2 with K1 only where finished groups appear long before the GEMM ends (several waves of
     // tiles): a one- or two-wave GEMM has nothing to hide behind, and the lean register budget and
     // the polling finalize warps then cost more than the early launch saves (measured).
     // (While the profiling events are recorded the SAME kernels run, but K2 is launched strictly after K1 so
     // that each has a duration of its own.)
-    const bool overlap = !up && c->overlap && (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
+    const bool overlap = !up && !split && c->overlap && (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
     gp.ready = overlap ? c->ready : nullptr;
     gp.V = c->V;
     gp.probe = c->probe; gp.probe_sink = reinterpret_cast<uint32_t*>(c->err + 1);
     gp.split_tma = gp.num_tiles < kOverlapMinWaves * workers ? 1 : 0;
-    // weights are streamed (read by one CTA when there is a single row block); hidden is re-read by every CTA
-    gp.policy_w = nrb == 1 ? kEvictFirst : kEvictNormal;
+    gp.split_k = split ? 2 : 1;
+    // weights are streamed (read by one CTA when there is a single row block) — unless the whole head is small enough to
+    // stay in L2 from one step to the next; hidden is re-read by every CTA
+    gp.policy_w = (nrb == 1 && static_cast<size_t>(c->NT) * c->d * 2 > (96u << 20)) ? kEvictFirst : kEvictNormal;
     gp.policy_h = kEvictLast;
-    const int grid = pair ? 2 * workers : workers;
+    const int grid = split ? 4 * workers : pair ? 2 * workers : workers;
 #ifdef CFGMS_TRACE
     gp.trace = c->trace_k1;
 #endif
@@ -438,8 +466,8 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
             gp.row0 = row0; gp.R = rows; gp.num_row_blocks = 1;
             gp.num_tiles = pair ? (gp.num_vocab_tiles + 1) / 2 : gp.num_vocab_tiles;
         }
-        const int launch_workers = std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
-        const int launch_grid = pair ? 2 * launch_workers : launch_workers;
+        const int launch_workers = split ? gp.num_tiles : std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
+        const int launch_grid = split ? 4 * launch_workers : pair ? 2 * launch_workers : launch_workers;
         using KernelFn = void (*)(const CUtensorMap, const CUtensorMap, const GemmParams);
         static const KernelFn table[8] = {
             cfgms_head_gemm_kernel<false, false, false>, cfgms_head_gemm_kernel<true, false, false>,
@@ -448,7 +476,10 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
             cfgms_head_gemm_kernel<false, true, true>,   cfgms_head_gemm_kernel<true, true, true>};
         static const KernelFn lean[4] = {cfgms_head_gemm_lean_kernel<false, false>, cfgms_head_gemm_lean_kernel<true, false>,
                                          cfgms_head_gemm_lean_kernel<false, true>, cfgms_head_gemm_lean_kernel<true, true>};
-        const KernelFn fn = overlap ? lean[(a->logits_out ? 1 : 0) | (pair ? 2 : 0)]
+        static const KernelFn splitk[4] = {cfgms_head_gemm_splitk_kernel<false, false>, cfgms_head_gemm_splitk_kernel<true, false>,
+                                           cfgms_head_gemm_splitk_kernel<false, true>, cfgms_head_gemm_splitk_kernel<true, true>};
+        const KernelFn fn = split ? splitk[(a->logits_out ? 1 : 0) | (c->use_cand ? 2 : 0)]
+                          : overlap ? lean[(a->logits_out ? 1 : 0) | (pair ? 2 : 0)]
                                     : table[(a->logits_out ? 1 : 0) | (c->use_cand ? 2 : 0) | (pair ? 4 : 0)];
         cudaLaunchConfig_t lc{};
         lc.gridDim = dim3(static_cast<unsigned>(launch_grid));
@@ -457,7 +488,7 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
         lc.stream = st;
         cudaLaunchAttribute attr[2];
         attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = pair ? 2 : 1;
+        attr[0].val.clusterDim.x = split ? 4 : pair ? 2 : 1;
         attr[0].val.clusterDim.y = 1;
         attr[0].val.clusterDim.z = 1;
         // the GEMM may be launched while the previous kernel of the stream still runs (it waits for it on the
@@ -559,6 +590,7 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     if (cudaPeekAtLastError() != cudaSuccess) return CFGMS_ERR_CUDA;
     c->info.row_tile = BN; c->info.row_blocks = nrb; c->info.gemm_grid = grid; c->info.pipeline_stages = stages;
     c->info.cta_pair = pair ? 1 : 0;
+    c->info.split_k = split ? 2 : 1;
     c->info.overlap = (overlap && !prof) ? 1 : 0;
     c->info.launches_last_step = launches;
     c->info.launches_total += launches;

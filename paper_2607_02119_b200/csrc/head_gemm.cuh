@@ -81,6 +81,7 @@ struct GemmParams {
     int* ready;          // nullable [S][num_row_blocks]: epilogue-warp arrivals per (stream, row block), see K2
     int V;               // tokens per stream (ready != nullptr requires V % kBM == 0)
     int split_tma;       // 1: warp 2 issues the row-tile loads; 0: warp 0 issues both (warp 2 idles)
+    int split_k;         // 1, or 2: one-wave GEMMs run on four-CTA clusters, two CTA pairs each taking half of K (kSplit build)
     // Measurement probes for the two design choices DESIGN.md section 7 argues (never set by default):
     //   probe bit 0: draw the Philox-Gumbel noise of EVERY merged logit in this epilogue (north_star's literal
     //                fusion) — the draws are folded into a sink word, results are unchanged: a lower bound of what
@@ -176,7 +177,46 @@ __device__ __forceinline__ void chunk_top4(const float* col, float (&val)[4], ui
           (static_cast<uint32_t>(ix[3]) << 24);
 }
 
-template <bool kTap, bool kCand, bool kPair>
+// The same selection by TWO lanes per request (split-K epilogue: a warp owns 16 requests x 32 tokens): lane
+// `part` (0 / 1) scans tokens [16 part, 16 part + 16) of the request's chunk, the two sorted packed-key lists are
+// merged through one shuffle each (the four largest of two descending lists a, b are max(a[i], b[3 - i]); packed
+// keys are distinct inside a chunk), and both lanes finish with the chunk's result.  Every lane of the warp calls it.
+__device__ __forceinline__ void chunk_top4_two_lanes(const float* col, int part, float (&val)[4], uint32_t& src) {
+    uint32_t t0 = 0u, t1 = 0u, t2 = 0u, t3 = 0u;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int idx = 16 * part + e;
+        const uint32_t u = __float_as_uint(col[idx]);
+        const uint32_t s = static_cast<uint32_t>(static_cast<int32_t>(u) >> 31);
+        uint32_t pk = ((u ^ (s | 0x80000000u)) | 31u) ^ static_cast<uint32_t>(idx);
+        uint32_t m;
+        m = min(t0, pk); t0 = max(t0, pk); pk = m;
+        m = min(t1, pk); t1 = max(t1, pk); pk = m;
+        m = min(t2, pk); t2 = max(t2, pk); pk = m;
+        t3 = max(t3, pk);
+    }
+    const uint32_t b0 = __shfl_xor_sync(0xffffffffu, t0, 16), b1 = __shfl_xor_sync(0xffffffffu, t1, 16);
+    const uint32_t b2 = __shfl_xor_sync(0xffffffffu, t2, 16), b3 = __shfl_xor_sync(0xffffffffu, t3, 16);
+    uint32_t c0 = max(t0, b3), c1 = max(t1, b2), c2 = max(t2, b1), c3 = max(t3, b0);
+    int ix[4] = {static_cast<int>((c0 & 31u) ^ 31u), static_cast<int>((c1 & 31u) ^ 31u),
+                 static_cast<int>((c2 & 31u) ^ 31u), static_cast<int>((c3 & 31u) ^ 31u)};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) val[j] = col[ix[j]];
+    // exact order: value descending, token ascending (the four are an unordered set here: full 4-sorter, then
+    // one more exchange of the middle pair is already part of the 5-comparator network)
+#define CFGMS_CX(a, b)                                                                   \
+    {                                                                                    \
+        const bool sw = (val[b] > val[a]) || (val[b] == val[a] && ix[b] < ix[a]);        \
+        const float tv = sw ? val[b] : val[a]; val[b] = sw ? val[a] : val[b]; val[a] = tv; \
+        const int ti = sw ? ix[b] : ix[a];    ix[b] = sw ? ix[a] : ix[b];    ix[a] = ti; \
+    }
+    CFGMS_CX(0, 1) CFGMS_CX(2, 3) CFGMS_CX(0, 2) CFGMS_CX(1, 3) CFGMS_CX(1, 2)
+#undef CFGMS_CX
+    src = static_cast<uint32_t>(ix[0]) | (static_cast<uint32_t>(ix[1]) << 8) | (static_cast<uint32_t>(ix[2]) << 16) |
+          (static_cast<uint32_t>(ix[3]) << 24);
+}
+
+template <bool kTap, bool kCand, bool kPair, bool kSplit = false>
 __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const CUtensorMap& tmap_h, const GemmParams& p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -190,12 +230,13 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     const uint32_t smem_coef_a = smem_b + stages * b_bytes;
     const uint32_t smem_coef_b = smem_coef_a + kCoefSlots * sizeof(SlotCoefA);
     const uint32_t bar_base = smem_coef_b + kCoefSlots * sizeof(SlotCoefB);
-    // barriers: full[8] | empty[8] | tmem_full[2] | tmem_empty[2] | tmem base pointer   (8 B each)
+    // barriers: full[8] | empty[8] | tmem_full[2] | tmem_empty[2] | tmem base pointer | 8 B spare | xchg[8]   (8 B each)
     const uint32_t bar_full = bar_base;
     const uint32_t bar_empty = bar_base + 8 * kMaxStages;
     const uint32_t bar_tfull = bar_base + 16 * kMaxStages;
     const uint32_t bar_tempty = bar_tfull + 16;
     const uint32_t tmem_ptr_smem = bar_tempty + 16;
+    const uint32_t bar_xchg = bar_tempty + 32;        // split-K: one per epilogue warp (partial sums received)
     const uint32_t smem_stg = bar_base + 256;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
     SlotCoefA* coef_a = reinterpret_cast<SlotCoefA*>(smem_gen + (smem_coef_a - smem_base));
@@ -204,10 +245,21 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const uint32_t cta_rank = kPair ? cluster_ctarank() : 0u;
+    // Cluster layout: one CTA; or a CTA pair (ranks 0, 1); or, split-K, two pairs (ranks 0, 1 | 2, 3) that work on the
+    // same tile, pair `ks` taking K blocks [ks * kb_half, (ks + 1) * kb_half).
+    static_assert(!kSplit || kPair, "split-K runs on CTA pairs");
+    const uint32_t cluster_rank = kPair ? cluster_ctarank() : 0u;
+    const uint32_t cta_rank = cluster_rank & 1u;              // rank inside the pair
+    const uint32_t leader_rank = cluster_rank & ~1u;          // cluster rank of this pair's leader
+    const uint16_t pair_mask = static_cast<uint16_t>(3u << leader_rank);
+    const int ks = kSplit ? static_cast<int>(cluster_rank >> 1) : 0;
     const bool leader = cta_rank == 0u;
-    const int worker = kPair ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
-    const int num_workers = kPair ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
+    const int cta_shift = kSplit ? 2 : kPair ? 1 : 0;
+    const int worker = static_cast<int>(blockIdx.x >> cta_shift);
+    const int num_workers = static_cast<int>(gridDim.x >> cta_shift);
+    const int kb_half = kSplit ? (p.num_kb + 1) >> 1 : p.num_kb;
+    const int kb_begin = ks * kb_half;
+    const int kb_end = min(p.num_kb, kb_begin + kb_half);
 
     if (threadIdx.x == 0) { CFGMS_TRACE_MARK(p.trace, 0); CFGMS_TRACE_MARK(p.trace, 1); }
     if (warp == 0 && lane == 0) {
@@ -221,6 +273,8 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             mbar_init(bar_tfull + 8 * a, 1);
             mbar_init(bar_tempty + 8 * a, kEpiWarps * (kPair ? 2 : 1));
         }
+        if (kSplit)
+            for (int w = 0; w < kEpiWarps; ++w) mbar_init(bar_xchg + 8 * w, 1);
         fence_barrier_init();
     }
     if (warp == 1) {
@@ -253,7 +307,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         const bool load_h = warp == 2 || !p.split_tma;
         if (load_h) pdl_wait_primary();        // the hidden states may come from the preceding kernel
         if (load_h && lane == 0) CFGMS_TRACE_MARK(p.trace, 3);   // previous kernel done (row producer)
-        const uint32_t full_sig = kPair ? mapa_shared(bar_full, 0u) : bar_full;
+        const uint32_t full_sig = kPair ? mapa_shared(bar_full, leader_rank) : bar_full;
         const uint32_t tx_bytes = (a_bytes + b_bytes) * (kPair ? 2u : 1u);
         int s = 0;
         uint32_t phase = 0;
@@ -262,7 +316,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             const int vp = tile / p.num_row_blocks;
             const int vt = kPair ? vp * 2 + static_cast<int>(cta_rank) : vp;
             const int row0 = rb * BN + static_cast<int>(cta_rank) * b_rows;
-            for (int kb = 0; kb < p.num_kb; ++kb) {
+            for (int kb = kb_begin; kb < kb_end; ++kb) {
                 mbar_wait(bar_empty + 8 * s, phase ^ 1, p.err, 1);
                 if (elect_one()) {
                     if (load_w) {
@@ -295,12 +349,12 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 mbar_wait(bar_tempty + 8 * acc, acc_phase ^ 1, p.err, 2);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * BN;
-                for (int kb = 0; kb < p.num_kb; ++kb) {
+                for (int kb = kb_begin; kb < kb_end; ++kb) {
                     mbar_wait(bar_full + 8 * s, phase, p.err, 3);
                     tc_fence_after();
-                    if (lane == 0 && tile == worker && kb == 0) CFGMS_TRACE_MARK(p.trace, 4);            // first stage landed
-                    if (lane == 0 && tile == worker && kb == p.num_kb / 2) CFGMS_TRACE_MARK(p.trace, 5); // half of the first tile
-                    if (lane == 0 && tile == worker && kb == p.num_kb - 1) CFGMS_TRACE_MARK(p.trace, 6); // last stage of the first tile landed
+                    if (lane == 0 && tile == worker && kb == kb_begin) CFGMS_TRACE_MARK(p.trace, 4);                  // first stage landed
+                    if (lane == 0 && tile == worker && kb == (kb_begin + kb_end) / 2) CFGMS_TRACE_MARK(p.trace, 5);   // half of the first tile
+                    if (lane == 0 && tile == worker && kb == kb_end - 1) CFGMS_TRACE_MARK(p.trace, 6);                // last stage of the first tile landed
                     if (elect_one()) {
                         // the start-address field counts 16-byte units
                         const uint64_t a_desc = a_desc0 + static_cast<uint64_t>((s * a_bytes) >> 4);
@@ -308,12 +362,13 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
 #pragma unroll
                         for (int k = 0; k < kBK / 16; ++k) {
                             // advance 16 bf16 = 32 B along K inside the swizzle span: +2 in the >>4 field
-                            if (kPair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
-                            else umma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0 ? 1u : 0u);
+                            const uint32_t accum = (kb != kb_begin || k != 0) ? 1u : 0u;
+                            if (kPair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, accum);
+                            else umma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, accum);
                         }
-                        if (kPair) umma_commit_pair(bar_empty + 8 * s); else umma_commit(bar_empty + 8 * s);
-                        if (kb == p.num_kb - 1) {
-                            if (kPair) umma_commit_pair(bar_tfull + 8 * acc); else umma_commit(bar_tfull + 8 * acc);
+                        if (kPair) umma_commit_pair(bar_empty + 8 * s, pair_mask); else umma_commit(bar_empty + 8 * s);
+                        if (kb == kb_end - 1) {
+                            if (kPair) umma_commit_pair(bar_tfull + 8 * acc, pair_mask); else umma_commit(bar_tfull + 8 * acc);
                         }
                     }
                     __syncwarp();
@@ -322,6 +377,138 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 if (++acc == 2) { acc = 0; acc_phase ^= 1; }
             }
         }
+    } else if (kSplit) {
+        // ================= split-K epilogue (warps 3..10, every CTA): one tile per cluster ============================
+        // The pair of K half `ks` OWNS batch columns [64 ks, 64 ks + 64) of the 128-column tile.  Epilogue warp
+        // (quarter, half) hands the 32 columns [64 (1 - ks) + 32 half, + 32) of its TMEM lane quarter to the same warp
+        // of the CTA that holds the same vocabulary rows in the other pair (cluster rank ^ 2) and finishes its own 32
+        // columns, so the eight warps of all four CTAs share the epilogue evenly.  The partial sums travel as
+        // asynchronous DSMEM stores into the receiving warp's (still unused) transpose stage and complete on that
+        // warp's own mbarrier: no cluster-wide barrier, no fence, and nothing touches a TMA ring that may still be busy.
+        const int ew = warp - kCtrlWarps;
+        const int quarter = warp & 3;
+        const int half = ew >> 2;
+        const int et = ew * 32 + lane;
+        const uint32_t xbar = bar_xchg + 8 * ew;
+        if (lane == 0) mbar_arrive_expect_tx(xbar, 4096);
+        pdl_wait_primary();
+        pdl_launch_dependents();
+        for (int slot = et; slot < p.num_row_blocks * (BN / 2); slot += 32 * kEpiWarps) {   // the host guarantees it fits
+            SlotCoefA ca; SlotCoefB cb;
+            make_slot_coef(p, p.row0 + 2 * slot, ca, cb);
+            coef_a[slot] = ca; coef_b[slot] = cb;
+        }
+        const int tile = worker;
+        const int rb = tile % p.num_row_blocks;
+        const int vt = (tile / p.num_row_blocks) * 2 + static_cast<int>(cta_rank);
+        const int col0 = 64 * ks + 32 * half;                 // first owned column of this warp
+        const int nb = vt * kBM + quarter * 32;               // first token of this warp's chunk
+        const int n = nb + lane;
+        const bool n_ok = n < p.NT;
+        const bool chunk_ok = nb < p.NT;
+        const float bias = n_ok ? __ldg(p.bias + n) : 0.f;
+        named_bar_sync(1, 32 * kEpiWarps);
+        mbar_wait(bar_tfull, 0, p.err, 4);
+        tc_fence_after();
+        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 7);
+        const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16);
+        const uint32_t stg_addr = smem_stg + static_cast<uint32_t>(ew) * (32 * kStgPitch * 4);
+        float* stg = reinterpret_cast<float*>(smem_gen + (stg_addr - smem_base));
+        uint32_t v[32];
+        {
+            uint32_t xs[32];
+            tmem_ld_32x32b_x32(taddr + 64 * (1 - ks) + 32 * half, xs);
+            tmem_ld_wait();
+            tmem_ld_32x32b_x32(taddr + col0, v);
+            const uint32_t dst = mapa_shared(stg_addr + static_cast<uint32_t>(lane) * 16u, cluster_rank ^ 2u);   // [col / 4][lane][4]
+            const uint32_t dbar = mapa_shared(xbar, cluster_rank ^ 2u);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                st_async_cluster_v4(dst + 512u * j, xs[4 * j], xs[4 * j + 1], xs[4 * j + 2], xs[4 * j + 3], dbar);
+            tmem_ld_wait();
+        }
+        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 12);     // partial sums sent
+        const size_t NT = static_cast<size_t>(p.NT);
+        const int row_base = p.row0 + rb * BN + col0;
+        const SlotCoefA* ca = coef_a + rb * (BN / 2) + (col0 >> 1);
+        const SlotCoefB* cb = coef_b + rb * (BN / 2) + (col0 >> 1);
+        SlotCoefA c[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) c[j] = ca[j];
+        mbar_wait_cluster(xbar, 0, p.err, 5);
+        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 13);     // partner's partial sums landed
+        {
+            const float4* rx = reinterpret_cast<const float4*>(stg) + lane;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float4 r = rx[32 * j];
+                v[4 * j] = __float_as_uint(__uint_as_float(v[4 * j]) + r.x);
+                v[4 * j + 1] = __float_as_uint(__uint_as_float(v[4 * j + 1]) + r.y);
+                v[4 * j + 2] = __float_as_uint(__uint_as_float(v[4 * j + 2]) + r.z);
+                v[4 * j + 3] = __float_as_uint(__uint_as_float(v[4 * j + 3]) + r.w);
+            }
+        }
+        __syncwarp();                                             // the stage is reused for the transpose below
+        char* zp = reinterpret_cast<char*>(p.z + static_cast<size_t>(row_base) * NT + n);
+        float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
+        const size_t row_stride = 2 * NT * sizeof(float);         // bytes between the even rows of two slots
+        const bool spill = n_ok && !(p.probe & 2);
+        const int o = lane & 15, part = lane >> 4;                // candidate pass: request o of the warp's 16, token half `part`
+        int any_kind = 0;
+        {   // the request at the even row of every slot: branch-free (predicated stores, running row pointer)
+            char* zq = zp;
+            asm volatile("" : "+l"(zq));
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const float a0 = __uint_as_float(v[2 * j]), a1 = __uint_as_float(v[2 * j + 1]);
+                const float z0 = fmaf(c[j].c00, a0, fmaf(c[j].c01, a1, bias * c[j].d0));
+                const bool own = (c[j].kind & 1) != 0;
+                any_kind |= c[j].kind;
+                st_global_f32_if(zq, z0, own && spill);
+                zq += row_stride;
+                if (kTap && own && n_ok) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
+                if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z0 + 0.0f : -INFINITY;
+            }
+        }
+        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 14);     // merge + z stores issued
+        if (kCand) {
+            __syncwarp();
+            float val[4]; uint32_t src;
+            chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
+            if ((ca[o].kind & 1) && chunk_ok && part == 0) {
+                const size_t chunk = (static_cast<size_t>(row_base + 2 * o) * NT + nb) >> 5;
+                *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
+                p.cand_src[chunk] = src;
+            }
+            __syncwarp();
+        }
+        if (any_kind & 2) {                                       // slots of two unpaired rows: the request at the odd row
+            char* zq = zp + NT * sizeof(float);
+            asm volatile("" : "+l"(zq));
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const SlotCoefB t = cb[j];
+                const float a1 = __uint_as_float(v[2 * j + 1]);
+                const float z1 = fmaf(t.c11, a1, bias * t.d1);
+                const bool own = (c[j].kind & 2) != 0;
+                st_global_f32_if(zq, z1, own && spill);
+                zq += row_stride;
+                if (kTap && own && n_ok) tp[static_cast<size_t>(2 * j + 1) * NT] = a1 + bias;
+                if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z1 + 0.0f : -INFINITY;
+            }
+            if (kCand) {
+                __syncwarp();
+                float val[4]; uint32_t src;
+                chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
+                if ((ca[o].kind & 2) && chunk_ok && part == 0) {
+                    const size_t chunk = (static_cast<size_t>(row_base + 2 * o + 1) * NT + nb) >> 5;
+                    *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
+                    p.cand_src[chunk] = src;
+                }
+                __syncwarp();
+            }
+        }
+        if (warp == kCtrlWarps && lane == 0) { CFGMS_TRACE_MARK(p.trace, 8); CFGMS_TRACE_MARK(p.trace, 9); }
     } else {
         // ================= epilogue (warps 3..10, every CTA) =================
         // batch parameters are read and z / candidates / counters written from here on
@@ -342,7 +529,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         const int nsp = BN / 64;                  // 64-column slab pairs per tile
         const int slots_per_rb = BN / 2;
         const bool full_table = p.num_row_blocks * slots_per_rb <= kCoefSlots;
-        const uint32_t tempty_sig = (kPair && !leader) ? mapa_shared(bar_tempty, 0u) : bar_tempty;
+        const uint32_t tempty_sig = (kPair && !leader) ? mapa_shared(bar_tempty, leader_rank) : bar_tempty;
         const size_t NT = static_cast<size_t>(p.NT);
         if (full_table) {
             // coefficients of every slot, once (the first mainloop hides it)
@@ -494,7 +681,10 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
     }
 
     tc_fence_before();
-    if (kPair) cluster_sync_all(); else __syncthreads();
+    // (split-K: nothing is published through this barrier — it keeps the four CTAs alive until every one of them has
+    // received its partner's partial sums and is done with the pair's tensor memory — so it carries no release fence,
+    // which would wait for the logit stores above to drain)
+    if (kSplit) cluster_sync_relaxed(); else if (kPair) cluster_sync_all(); else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
         if (kPair) tmem_dealloc_pair(tmem_base, kTmemCols); else tmem_dealloc(tmem_base, kTmemCols);
@@ -508,6 +698,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1)
 cfgms_head_gemm_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
                        const GemmParams p) {
     head_gemm_body<kTap, kCand, kPair>(tmap_w, tmap_h, p);
+}
+
+// Split-K build for one-wave GEMMs (clusters of four CTAs; the host chooses it, see choose_row_tile in cfgms.cu).
+template <bool kTap, bool kCand>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+cfgms_head_gemm_splitk_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_h,
+                              const GemmParams p) {
+    head_gemm_body<kTap, kCand, true, true>(tmap_w, tmap_h, p);
 }
 
 // Lean register budget (see "Register budget" above): leaves room for the finalize kernel's CTAs on

@@ -202,11 +202,55 @@ __device__ __forceinline__ void umma_bf16_pair(uint32_t d_tmem, uint64_t a_desc,
 }
 // Arrive on the mbarrier at the same shared-memory offset in BOTH CTAs of the pair once all
 // tcgen05.mma issued so far have completed.
-__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+// (`cta_mask`: the two cluster ranks of the pair, 3 for ranks 0 and 1, 0xC for ranks 2 and 3 of a four-CTA cluster.)
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar, uint16_t cta_mask = 3) {
     asm volatile(
         "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-        ::"r"(bar), "h"(static_cast<uint16_t>(3))
+        ::"r"(bar), "h"(cta_mask)
         : "memory");
+}
+// 16-byte asynchronous store into the shared memory of another CTA of the cluster; its completion is counted (16
+// transaction bytes) on an mbarrier of THAT CTA, so the receiver needs no fence and no cluster-wide barrier: it
+// waits on its own mbarrier.  Both addresses are shared::cluster addresses (mapa_shared) of the same target CTA.
+__device__ __forceinline__ void st_async_cluster_v4(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d,
+                                                    uint32_t cluster_bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(cluster_addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(cluster_bar)
+                 : "memory");
+}
+// Wait for a phase whose transactions were written by another CTA of the cluster (acquire at cluster scope); bounded.
+__device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity, int* err, int tag) {
+    const uint64_t t0 = global_timer_ns();
+    uint32_t spins = 0;
+    while (!mbar_try_wait_cluster(bar, parity)) {
+        if ((++spins & 0x3ffu) == 0 && global_timer_ns() - t0 > 2000000000ull) {
+            if (err) atomicCAS(err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (tag << 8));
+            __threadfence_system();
+            __trap();
+        }
+    }
+}
+// Cluster barrier without the release fence (nothing is published through it: it only keeps every CTA of the
+// cluster alive until all of them are done with each other's shared memory and tensor memory).
+__device__ __forceinline__ void cluster_sync_relaxed() {
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// Predicated streaming store (no branch: keeps an unrolled epilogue loop free of control flow).
+__device__ __forceinline__ void st_global_f32_if(void* p, float v, bool pred) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t@q st.global.cs.f32 [%0], %1;\n\t}"
+                 ::"l"(p), "f"(v), "r"(static_cast<int>(pred)) : "memory");
 }
 
 // TMEM -> registers: 32 lanes x 32 consecutive 32-bit columns; thread t of the warp gets lane
