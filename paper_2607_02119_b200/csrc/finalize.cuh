@@ -916,11 +916,20 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                 __syncwarp();
                 CFGMS_K2_MARK(6);  // overflow chunks handled, exact threshold known
                 if (n_list >= 0) {
-                    for (int e = lane; e < n_list; e += 32) {
-                        const uint32_t ck = list_key[e];
-                        if (ck >= thr) {
-                            const int v = list_v[e];
-                            best_update(best, greedy ? key_float(ck) : key_float(ck) + gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, v), v);
+                    // two list entries per lane and iteration, so that their Philox / logarithm chains overlap
+                    for (int e = lane; e < n_list; e += 64) {
+                        const int e2 = e + 32 < n_list ? e + 32 : e;
+                        const uint32_t ka = list_key[e], kb = list_key[e2];
+                        const int va = list_v[e], vb = list_v[e2];
+                        const bool sa = ka >= thr, sb = e2 != e && kb >= thr;
+                        if (greedy) {
+                            if (sa) best_update(best, key_float(ka), va);
+                            if (sb) best_update(best, key_float(kb), vb);
+                        } else if (sa || sb) {
+                            const float ga = gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, va);
+                            const float gb = gumbel_noise(p.seed_lo, p.seed_hi, req, tau, gi, vb);
+                            if (sa) best_update(best, key_float(ka) + ga, va);
+                            if (sb) best_update(best, key_float(kb) + gb, vb);
                         }
                     }
                 } else {
@@ -949,6 +958,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     if (valid && lane == 0) write_cell(p, r, i, pm, cp, token, modality);
     xchg_finish(p);
     CFGMS_K2_MARK(8);
+    CFGMS_K2_MARK(15);
     if (p.ready) {
         // the last CTA to finish re-arms the counters for the next step's K1 (which starts after this grid)
         __syncthreads();

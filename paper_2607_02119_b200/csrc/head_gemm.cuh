@@ -401,7 +401,13 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         const int tile = worker;
         const int rb = tile % p.num_row_blocks;
         const int vt = (tile / p.num_row_blocks) * 2 + static_cast<int>(cta_rank);
-        const int col0 = 64 * ks + 32 * half;                 // first owned column of this warp
+        // Batches of at most 64 rows fill only columns [0, 64): there the pair of K half `ks` owns the 32 columns
+        // [32 ks, 32 ks + 32) and its two warps per lane quarter split the two passes over them (half 0: the requests
+        // at even rows, half 1: those at odd rows of unpaired slots), so that a CFG-off batch does not leave one pair
+        // idle while the other runs both passes.
+        const bool narrow = p.R <= 64;
+        const int col0 = narrow ? 32 * ks : 64 * ks + 32 * half;                 // first owned column of this warp
+        const int send_col = narrow ? 32 * (1 - ks) : 64 * (1 - ks) + 32 * half; // first column handed to the other pair
         const int nb = vt * kBM + quarter * 32;               // first token of this warp's chunk
         const int n = nb + lane;
         const bool n_ok = n < p.NT;
@@ -417,7 +423,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         uint32_t v[32];
         {
             uint32_t xs[32];
-            tmem_ld_32x32b_x32(taddr + 64 * (1 - ks) + 32 * half, xs);
+            tmem_ld_32x32b_x32(taddr + send_col, xs);
             tmem_ld_wait();
             tmem_ld_32x32b_x32(taddr + col0, v);
             const uint32_t dst = mapa_shared(stg_addr + static_cast<uint32_t>(lane) * 16u, cluster_rank ^ 2u);   // [col / 4][lane][4]
@@ -455,7 +461,11 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         const bool spill = n_ok && !(p.probe & 2);
         const int o = lane & 15, part = lane >> 4;                // candidate pass: request o of the warp's 16, token half `part`
         int any_kind = 0;
-        {   // the request at the even row of every slot: branch-free (predicated stores, running row pointer)
+#pragma unroll
+        for (int j = 0; j < 16; ++j) any_kind |= c[j].kind;
+        const bool pass_a = !narrow || half == 0;
+        const bool pass_b = (any_kind & 2) != 0 && (!narrow || half == 1);
+        if (pass_a) {   // the request at the even row of every slot: branch-free (predicated stores, running row pointer)
             char* zq = zp;
             asm volatile("" : "+l"(zq));
 #pragma unroll
@@ -463,7 +473,6 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 const float a0 = __uint_as_float(v[2 * j]), a1 = __uint_as_float(v[2 * j + 1]);
                 const float z0 = fmaf(c[j].c00, a0, fmaf(c[j].c01, a1, bias * c[j].d0));
                 const bool own = (c[j].kind & 1) != 0;
-                any_kind |= c[j].kind;
                 st_global_f32_if(zq, z0, own && spill);
                 zq += row_stride;
                 if (kTap && own && n_ok) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
@@ -471,7 +480,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             }
         }
         if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 14);     // merge + z stores issued
-        if (kCand) {
+        if (kCand && pass_a) {
             __syncwarp();
             float val[4]; uint32_t src;
             chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
@@ -482,7 +491,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             }
             __syncwarp();
         }
-        if (any_kind & 2) {                                       // slots of two unpaired rows: the request at the odd row
+        if (pass_b) {                                             // slots of two unpaired rows: the request at the odd row
             char* zq = zp + NT * sizeof(float);
             asm volatile("" : "+l"(zq));
 #pragma unroll
@@ -689,7 +698,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         tc_fence_after();
         if (kPair) tmem_dealloc_pair(tmem_base, kTmemCols); else tmem_dealloc(tmem_base, kTmemCols);
     }
-    if (threadIdx.x == 0) CFGMS_TRACE_MARK(p.trace, 10);
+    if (threadIdx.x == 0) { CFGMS_TRACE_MARK(p.trace, 10); CFGMS_TRACE_MARK(p.trace, 15); }
 }
 
 // Full register budget (168): the fastest GEMM, but nothing else fits on its SMs while it runs.

@@ -301,7 +301,7 @@ __device__ __forceinline__ void st_global_f32(void* p, float v) {
 // slot 0 of a CTA's 16-word record holds %globaltimer at entry, slots 1.. hold %clock64 at the marks.
 #ifdef CFGMS_TRACE
 __device__ __forceinline__ void trace_mark(unsigned long long* trace, int slot) {
-    if (trace) trace[blockIdx.x * 16 + slot] = slot == 0 ? global_timer_ns() : static_cast<unsigned long long>(clock64());
+    if (trace) trace[blockIdx.x * 16 + slot] = (slot == 0 || slot == 15) ? global_timer_ns() : static_cast<unsigned long long>(clock64());
 }
 #define CFGMS_TRACE_MARK(trace, slot) trace_mark(trace, slot)
 #else
