@@ -522,7 +522,7 @@ def main():
                                    wl.heads.numel() * 2 / 2 ** 20, wl.hidden_pool.numel() * wl.hidden_pool.element_size() / 2 ** 20,
                                    wl.n_req * wl.S * wl.V * 4 / 2 ** 20),
                                row_tile=info["row_tile"], row_blocks=info["row_blocks"], gemm_grid=info["gemm_grid"],
-                               pipeline_stages=info["pipeline_stages"], cta_pair=bool(info["cta_pair"])),
+                               pipeline_stages=info["pipeline_stages"], cta_pair=bool(info["cta_pair"]), split_k=info["split_k"]),
                 "clocks": sampler.summary(), "gpu_launches": int((info["launches_last_step"] + (1 if sharded else 0)) * K + (0 if sharded else 1)),
                 "roofline": roof}
 
@@ -588,7 +588,8 @@ def main():
                                           "us_per_step_cold_l2_eager": cold_eager_us[0],
                                           "us_per_step_cold_l2_eager_p10_p90": [cold_eager_us[1], cold_eager_us[2]], "gemm_us": g_us,
                                           "finalize_us": f_us, "frames_per_s_hot": r.wl.n_req / hot_us * 1e6,
-                                          "roofline_us": t_roof, "frac_hot": t_roof / hot_us, "frac_cold": t_roof / cold_us}
+                                          "roofline_us": t_roof, "frac_hot": t_roof / hot_us, "frac_cold": t_roof / cold_us,
+                                          "split_k": r.ctx.info()["split_k"], "gemm_grid": r.ctx.info()["gemm_grid"]}
                 if cfg in (2, 3):
                     ro = Runner(cfg, dev, cfg_off=True)
                     ms_o = ro.time_graph(min(K, ro.wl.T), W, with_deint=False)

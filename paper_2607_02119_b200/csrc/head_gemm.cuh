@@ -603,6 +603,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                 // fixed stride so that the stores stay predicated (no per-row address rebuild, no branch).
                 const int own_even = n_ok ? 1 : 0, own_odd = n_ok ? 2 : 0;   // kind bits this thread may act on
                 const size_t row_stride = 2 * NT * sizeof(float);      // bytes between the even rows of two slots
+                const bool spill = !(p.probe & 2);
                 {
                     char* zq = reinterpret_cast<char*>(zp);
                     char* tq = reinterpret_cast<char*>(tp);
@@ -615,7 +616,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                         const float z0 = fmaf(c.c00, a0, fmaf(c.c01, a1, bias * c.d0));
                         const bool own = (c.kind & own_even) != 0;
                         any_odd |= c.kind;
-                        if (own && !(p.probe & 2)) st_global_f32(zq, z0);
+                        st_global_f32_if(zq, z0, own && spill);       // predicated, no branch: the unrolled loop pipelines
                         if (kTap) {
                             if (own) { const SlotCoefB t = cb[j]; *reinterpret_cast<float*>(tq) = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
                             tq += row_stride;
@@ -657,7 +658,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
                         const float a1 = __uint_as_float(v[2 * j + 1]);
                         const float z1 = fmaf(c.c11, a1, bias * c.d1);
                         const bool own = (kind & own_odd) != 0;
-                        if (own) st_global_f32(zq, z1);
+                        st_global_f32_if(zq, z1, own);
                         if (kTap) {
                             if (own) *reinterpret_cast<float*>(tq) = a1 + bias;
                             tq += row_stride;

@@ -22,7 +22,7 @@ LOGIT_TOL = 2e-2
 
 class DeviceWorkload:
     def __init__(self, wl: workloads.Workload, dev, T_cap=None, row_tile: int = 0, no_candidates: bool = False,
-                 no_overlap: bool = False, force_overlap: bool = False):
+                 no_overlap: bool = False, force_overlap: bool = False, **ctx_kwargs):
         import paper_2607_02119_b200 as pkg
         self.wl = wl
         self.dev = dev
@@ -30,7 +30,8 @@ class DeviceWorkload:
         self.heads = cu(wl.heads)
         self.embeds = cu(wl.embeds)
         self.ctx = pkg.Context(self.heads, self.embeds, max_rows=max(wl.R, 2), row_tile=row_tile,
-                               no_candidates=no_candidates, no_overlap=no_overlap, force_overlap=force_overlap)
+                               no_candidates=no_candidates, no_overlap=no_overlap, force_overlap=force_overlap,
+                               **ctx_kwargs)
         self.pool = cu(wl.hidden_pool)
         self.pair_map, self.w, self.temp, self.top_k = cu(wl.pair_map), cu(wl.w), cu(wl.temp), cu(wl.top_k)
         self.req_id, self.n_frames = cu(wl.req_id), cu(wl.n_frames)
