@@ -271,6 +271,45 @@ class Runner:
         both, alone = replay_ms(graph_of(True)), replay_ms(graph_of(False))
         return max(1e3 * (both - alone) / K, 0.0), eager
 
+    def time_deinterleave(self, flush, K: int = 20):
+        """K3 alone, cold: (graph of K x (L2 flush + cfgms_deinterleave of the full delayed buffer)) - (graph of K x flush).
+        -> (us per call, algorithmic bytes per call: every delayed cell read once, every grid cell written once)."""
+        torch = self.torch
+        wl = self.wl
+
+        def graph_of(with_k3: bool):
+            g = torch.cuda.CUDAGraph()
+            s = torch.cuda.Stream(device=self.dev)
+            s.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(s):
+                flush.add_(1)
+                self.deinterleave()
+            torch.cuda.current_stream().wait_stream(s)
+            torch.cuda.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                for _ in range(K):
+                    flush.add_(1)
+                    if with_k3:
+                        self.deinterleave()
+            return g
+
+        def replay_ms(g):
+            g.replay()
+            torch.cuda.synchronize()
+            best = None
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                g.replay()
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1)
+                best = ms if best is None else min(best, ms)
+            return best
+
+        us = max(1e3 * (replay_ms(graph_of(True)) - replay_ms(graph_of(False))) / K, 1e-3)
+        return us, 4.0 * wl.R * (wl.T + (wl.T - wl.S + 1)) * wl.S
+
     def time_widenings(self, K: int):
         """Widening kernels at this config: feedback gather-sum alone (CUDA
         events, tables larger than L2), and the step with streaming frame emission switched on."""
@@ -570,9 +609,13 @@ def main():
             wd = main_r.time_widenings(50)
             wd["feedback_frac_of_hbm_peak"] = wd["feedback_gbs"] / peaks["hbm_gbs"]
             line["widenings"] = wd
+            flush = torch.zeros(256 * 2 ** 20 // 4, dtype=torch.int32, device=dev)
+            k3_us, k3_bytes = main_r.time_deinterleave(flush)
+            line["deinterleave"] = {"kernel": "cfgms_deinterleave_kernel", "us_cold_l2": k3_us, "algorithmic_bytes": k3_bytes,
+                                    "gbs": k3_bytes / k3_us / 1e3, "frac_of_hbm_peak": k3_bytes / k3_us / 1e3 / peaks["hbm_gbs"],
+                                    "how": "graph of 20 x (256 MiB L2 flush + de-interleave of the full [rows][T][S] buffer) minus graph of 20 x flush"}
             del main_r
             torch.cuda.empty_cache()
-            flush = torch.zeros(256 * 2 ** 20 // 4, dtype=torch.int32, device=dev)
             extras = {}
             ratio = {}
             for cfg in (2, 3, 4):
