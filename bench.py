@@ -583,8 +583,8 @@ def main():
         link = main_r.pcie_h2d_gbs()
         line["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                        "us_per_step": 1e6 * dt_e2e / Ke,
-                       "api": "cfgms_step_host (pinned host buffers; hidden states uploaded row block by row block on a second "
-                              "stream while the GEMM of the previous block runs; sync per step)",
+                       "api": "cfgms_step_host (pinned host buffers; hidden states uploaded in two chunks of row blocks on a second "
+                              "stream, the second chunk under the GEMM of the first; sync per step)",
                        "host_link_h2d_gbs": link, "h2d_us_at_link_rate": h2d / link / 1e3}
 
     if rank == 0 and world == 1 and not sharded:

@@ -366,7 +366,7 @@ void cfgms_destroy(cfgms_ctx* c) {
 namespace {
 
 // Host-buffer mode of a step (cfgms_step_host): the hidden states are still in (pinned) host memory; they are
-// uploaded one GEMM row block at a time on a second stream while the GEMM of the previous row block runs.
+// uploaded in two chunks of GEMM row blocks on a second stream, the second chunk while the GEMM of the first runs.
 struct HostUpload {
     const char* host_hidden;   // bf16 [R][d] on the host
     char* dev_hidden;          // staging on the device
@@ -443,16 +443,19 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     const size_t smem = GemmSmemLayout::total(b_rows, stages);
     gp.row0 = 0;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
-    // One launch for the whole batch — or, in host-buffer mode, one launch per uploaded row block: block k + 1 crosses
-    // PCIe while the GEMM of block k runs (each launch re-streams the weights, which the tensor-bound regime hides).
-    const int n_launch = up ? nrb : 1;
+    // One launch for the whole batch — or, in host-buffer mode, one launch per uploaded chunk of row blocks: chunk k + 1
+    // crosses PCIe while the GEMM of chunk k runs.
+    // Two chunks: every launch streams the whole head once more, so fewer, larger launches win as long as the first GEMM
+    // can start before the upload ends (config 5, 8 MiB over PCIe: 361 us/step with two chunks, 390 with four, 423 with one).
+    const int cb = (nrb + 1) / 2;       // row blocks per uploaded chunk
+    const int n_launch = up ? (nrb + cb - 1) / cb : 1;
     if (n_launch > 15) return CFGMS_ERR_SHAPE;      // chunk events 0..14 (15 orders the copy stream behind the caller's)
     for (int k = 0; k < n_launch; ++k) {
         CUtensorMap tmap_chunk;
         const CUtensorMap* tmap_h = &c->tmap_h;
         if (up) {
             HostStage& hs = c->hs;
-            const int row0 = k * BN, rows = std::min(BN, a->R - row0);
+            const int row0 = k * cb * BN, rows = std::min(cb * BN, a->R - row0);
             const size_t off = static_cast<size_t>(row0) * c->d * 2, bytes = static_cast<size_t>(rows) * c->d * 2;
             if (cudaMemcpyAsync(up->dev_hidden + off, up->host_hidden + off, bytes, cudaMemcpyHostToDevice, hs.copy_stream) != cudaSuccess ||
                 cudaEventRecord(hs.chunk_ev[k], hs.copy_stream) != cudaSuccess ||
@@ -463,8 +466,8 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
                               static_cast<uint32_t>(b_rows));
             if (rc != CFGMS_OK) return rc;
             tmap_h = &tmap_chunk;
-            gp.row0 = row0; gp.R = rows; gp.num_row_blocks = 1;
-            gp.num_tiles = pair ? (gp.num_vocab_tiles + 1) / 2 : gp.num_vocab_tiles;
+            gp.row0 = row0; gp.R = rows; gp.num_row_blocks = (rows + BN - 1) / BN;
+            gp.num_tiles = (pair ? (gp.num_vocab_tiles + 1) / 2 : gp.num_vocab_tiles) * gp.num_row_blocks;
         }
         const int launch_workers = split ? gp.num_tiles : std::min(gp.num_tiles, pair ? c->num_sms / 2 : c->num_sms);
         const int launch_grid = split ? 4 * launch_workers : pair ? 2 * launch_workers : launch_workers;
@@ -662,8 +665,8 @@ int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     d.frame_index_out = a->frame_index_out ? h.frame_index : nullptr;
     d.hidden = h.hidden;
     if (a->hidden_dtype == CFGMS_BF16) {
-        // hidden states: uploaded row block by row block on the copy stream, each block's GEMM launch waits for its own
-        // block only (step_impl).  The copy stream first waits for whatever precedes this call on the caller's stream.
+        // hidden states: uploaded in two chunks on the copy stream, each chunk's GEMM launch waits for its own
+        // chunk only (step_impl).  The copy stream first waits for whatever precedes this call on the caller's stream.
         if (cudaEventRecord(h.chunk_ev[15], st) != cudaSuccess || cudaStreamWaitEvent(h.copy_stream, h.chunk_ev[15], 0) != cudaSuccess)
             return CFGMS_ERR_CUDA;
         HostUpload up{static_cast<const char*>(a->hidden), static_cast<char*>(h.hidden), &h2d};
