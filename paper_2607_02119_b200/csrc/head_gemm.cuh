@@ -140,44 +140,14 @@ __device__ __forceinline__ void make_slot_coef(const GemmParams& p, int r0, Slot
 
 // Per-chunk candidate pass (north_star step 3, "per-N-tile top-k candidate pass held in warp
 // registers").  The warp's 32 tokens x 32 requests block is transposed through a warp-private
-// shared-memory stage; afterwards lane o owns request o and the chunk's 32 z values.  It keeps
+// shared-memory stage; afterwards two lanes share a request's chunk of 32 z values.  They keep
 // the four largest as PACKED keys (order-preserving 27-bit float key | 5-bit reversed token
 // offset) with 7 integer min/max per value — no predicates, no index bookkeeping — then
 // re-reads the four exact values and emits them sorted (descending, lowest token first).
 // Selection granularity is the 27-bit key bucket: a value that is NOT emitted has
 //     float_key(hidden) <= float_key(smallest emitted) | 31,
 // which is the bound K2 uses to decide whether a chunk may hide a top-k member.
-__device__ __forceinline__ void chunk_top4(const float* col, float (&val)[4], uint32_t& src) {
-    uint32_t t0 = 0u, t1 = 0u, t2 = 0u, t3 = 0u;
-#pragma unroll
-    for (int e = 0; e < 32; ++e) {
-        const uint32_t u = __float_as_uint(col[e]);
-        const uint32_t s = static_cast<uint32_t>(static_cast<int32_t>(u) >> 31);
-        uint32_t pk = ((u ^ (s | 0x80000000u)) | 31u) ^ static_cast<uint32_t>(e);
-        uint32_t m;
-        m = min(t0, pk); t0 = max(t0, pk); pk = m;
-        m = min(t1, pk); t1 = max(t1, pk); pk = m;
-        m = min(t2, pk); t2 = max(t2, pk); pk = m;
-        t3 = max(t3, pk);
-    }
-    int ix[4] = {static_cast<int>((t0 & 31u) ^ 31u), static_cast<int>((t1 & 31u) ^ 31u),
-                 static_cast<int>((t2 & 31u) ^ 31u), static_cast<int>((t3 & 31u) ^ 31u)};
-#pragma unroll
-    for (int j = 0; j < 4; ++j) val[j] = col[ix[j]];
-    // exact order inside a bucket: value descending, token ascending (5-comparator network)
-#define CFGMS_CX(a, b)                                                                   \
-    {                                                                                    \
-        const bool sw = (val[b] > val[a]) || (val[b] == val[a] && ix[b] < ix[a]);        \
-        const float tv = sw ? val[b] : val[a]; val[b] = sw ? val[a] : val[b]; val[a] = tv; \
-        const int ti = sw ? ix[b] : ix[a];    ix[b] = sw ? ix[a] : ix[b];    ix[a] = ti; \
-    }
-    CFGMS_CX(0, 1) CFGMS_CX(2, 3) CFGMS_CX(0, 2) CFGMS_CX(1, 3) CFGMS_CX(1, 2)
-#undef CFGMS_CX
-    src = static_cast<uint32_t>(ix[0]) | (static_cast<uint32_t>(ix[1]) << 8) | (static_cast<uint32_t>(ix[2]) << 16) |
-          (static_cast<uint32_t>(ix[3]) << 24);
-}
-
-// The same selection by TWO lanes per request (split-K epilogue: a warp owns 16 requests x 32 tokens): lane
+// TWO lanes per request (a warp finishes 16 requests x 32 tokens per slab): lane
 // `part` (0 / 1) scans tokens [16 part, 16 part + 16) of the request's chunk, the two sorted packed-key lists are
 // merged through one shuffle each (the four largest of two descending lists a, b are max(a[i], b[3 - i]); packed
 // keys are distinct inside a chunk), and both lanes finish with the chunk's result.  Every lane of the warp calls it.
@@ -216,7 +186,91 @@ __device__ __forceinline__ void chunk_top4_two_lanes(const float* col, int part,
           (static_cast<uint32_t>(ix[3]) << 24);
 }
 
-template <bool kTap, bool kCand, bool kPair, bool kSplit = false>
+// One 32-column slab (16 two-row slots x 32 tokens: lane = token, v[2 j], v[2 j + 1] = the accumulators of slot j's two
+// rows) from accumulators to outputs: CFG merge + bias + 1 / temperature, the z spill, and the candidate pass (transpose
+// through `stg`, two lanes per request).  Pass A serves the request at the even row of every slot, pass B the request at
+// the odd row of slots that hold two unpaired rows.  Branch-free inner loops: predicated stores, one running row
+// pointer, coefficients preloaded by the caller — so the unrolled loops pipeline instead of serialising on a load, a
+// branch and a store per slot.
+template <bool kTap, bool kCand>
+__device__ __forceinline__ void finish_slab(const GemmParams& p, const uint32_t (&v)[32], const SlotCoefA (&c)[16],
+                                            const SlotCoefA* ca, const SlotCoefB* cb, float* stg, int row_base, int n, int nb,
+                                            bool n_ok, bool chunk_ok, float bias, int lane, bool allow_a, bool allow_b) {
+    const size_t NT = static_cast<size_t>(p.NT);
+    char* zp = reinterpret_cast<char*>(p.z + static_cast<size_t>(row_base) * NT + n);
+    float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
+    const size_t row_stride = 2 * NT * sizeof(float);         // bytes between the even rows of two slots
+    const bool spill = n_ok && !(p.probe & 2);
+    const int o = lane & 15, part = lane >> 4;                // candidate pass: request o of the warp's 16, token half `part`
+    int any_kind = 0;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) any_kind |= c[j].kind;
+    const bool pass_a = allow_a && (any_kind & 1) != 0;
+    const bool pass_b = allow_b && (any_kind & 2) != 0;
+    if (pass_a) {
+        char* zq = zp;
+        asm volatile("" : "+l"(zq));
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const float a0 = __uint_as_float(v[2 * j]), a1 = __uint_as_float(v[2 * j + 1]);
+            const float z0 = fmaf(c[j].c00, a0, fmaf(c[j].c01, a1, bias * c[j].d0));
+            const bool own = (c[j].kind & 1) != 0;
+            st_global_f32_if(zq, z0, own && spill);
+            zq += row_stride;
+            if (kTap && own && n_ok) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
+            if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z0 + 0.0f : -INFINITY;
+        }
+        if (kCand && (p.probe & 1)) {
+            // measurement probe: the noise of every merged logit of the slab, drawn here (rolled loop over the staged z
+            // values so that the product path's code stays as it is); the draws are folded into a sink word
+            uint32_t sink = 0u;
+#pragma unroll 1
+            for (int j = 0; j < 16; ++j)
+                sink ^= __float_as_uint(stg[j * kStgPitch + lane] +
+                                        gumbel_noise(0x1234u, 0x5678u, static_cast<uint32_t>(row_base + 2 * j), 7, n >> 11, n & 2047));
+            if (sink == 0x9e3779b9u) *p.probe_sink = sink;    // keeps the draws alive
+        }
+        if (kCand) {
+            __syncwarp();
+            float val[4]; uint32_t src;
+            chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
+            if ((ca[o].kind & 1) && chunk_ok && part == 0) {
+                const size_t chunk = (static_cast<size_t>(row_base + 2 * o) * NT + nb) >> 5;
+                *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
+                p.cand_src[chunk] = src;
+            }
+            __syncwarp();
+        }
+    }
+    if (pass_b) {
+        char* zq = zp + NT * sizeof(float);
+        asm volatile("" : "+l"(zq));
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const SlotCoefB t = cb[j];
+            const float a1 = __uint_as_float(v[2 * j + 1]);
+            const float z1 = fmaf(t.c11, a1, bias * t.d1);
+            const bool own = (c[j].kind & 2) != 0;
+            st_global_f32_if(zq, z1, own && spill);
+            zq += row_stride;
+            if (kTap && own && n_ok) tp[static_cast<size_t>(2 * j + 1) * NT] = a1 + bias;
+            if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z1 + 0.0f : -INFINITY;
+        }
+        if (kCand) {
+            __syncwarp();
+            float val[4]; uint32_t src;
+            chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
+            if ((ca[o].kind & 2) && chunk_ok && part == 0) {
+                const size_t chunk = (static_cast<size_t>(row_base + 2 * o + 1) * NT + nb) >> 5;
+                *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
+                p.cand_src[chunk] = src;
+            }
+            __syncwarp();
+        }
+    }
+}
+
+template <bool kTap, bool kCand, bool kPair, bool kSplit = false, int EW = kEpiWarps>
 __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const CUtensorMap& tmap_h, const GemmParams& p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -271,10 +325,10 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         }
         for (int a = 0; a < 2; ++a) {
             mbar_init(bar_tfull + 8 * a, 1);
-            mbar_init(bar_tempty + 8 * a, kEpiWarps * (kPair ? 2 : 1));
+            mbar_init(bar_tempty + 8 * a, EW * (kPair ? 2 : 1));
         }
         if (kSplit)
-            for (int w = 0; w < kEpiWarps; ++w) mbar_init(bar_xchg + 8 * w, 1);
+            for (int w = 0; w < EW; ++w) mbar_init(bar_xchg + 8 * w, 1);
         fence_barrier_init();
     }
     if (warp == 1) {
@@ -393,7 +447,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         if (lane == 0) mbar_arrive_expect_tx(xbar, 4096);
         pdl_wait_primary();
         pdl_launch_dependents();
-        for (int slot = et; slot < p.num_row_blocks * (BN / 2); slot += 32 * kEpiWarps) {   // the host guarantees it fits
+        for (int slot = et; slot < p.num_row_blocks * (BN / 2); slot += 32 * EW) {   // the host guarantees it fits
             SlotCoefA ca; SlotCoefB cb;
             make_slot_coef(p, p.row0 + 2 * slot, ca, cb);
             coef_a[slot] = ca; coef_b[slot] = cb;
@@ -413,7 +467,7 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
         const bool n_ok = n < p.NT;
         const bool chunk_ok = nb < p.NT;
         const float bias = n_ok ? __ldg(p.bias + n) : 0.f;
-        named_bar_sync(1, 32 * kEpiWarps);
+        named_bar_sync(1, 32 * EW);
         mbar_wait(bar_tfull, 0, p.err, 4);
         tc_fence_after();
         if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 7);
@@ -455,99 +509,34 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             }
         }
         __syncwarp();                                             // the stage is reused for the transpose below
-        char* zp = reinterpret_cast<char*>(p.z + static_cast<size_t>(row_base) * NT + n);
-        float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
-        const size_t row_stride = 2 * NT * sizeof(float);         // bytes between the even rows of two slots
-        const bool spill = n_ok && !(p.probe & 2);
-        const int o = lane & 15, part = lane >> 4;                // candidate pass: request o of the warp's 16, token half `part`
-        int any_kind = 0;
-#pragma unroll
-        for (int j = 0; j < 16; ++j) any_kind |= c[j].kind;
-        const bool pass_a = !narrow || half == 0;
-        const bool pass_b = (any_kind & 2) != 0 && (!narrow || half == 1);
-        if (pass_a) {   // the request at the even row of every slot: branch-free (predicated stores, running row pointer)
-            char* zq = zp;
-            asm volatile("" : "+l"(zq));
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const float a0 = __uint_as_float(v[2 * j]), a1 = __uint_as_float(v[2 * j + 1]);
-                const float z0 = fmaf(c[j].c00, a0, fmaf(c[j].c01, a1, bias * c[j].d0));
-                const bool own = (c[j].kind & 1) != 0;
-                st_global_f32_if(zq, z0, own && spill);
-                zq += row_stride;
-                if (kTap && own && n_ok) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
-                if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z0 + 0.0f : -INFINITY;
-            }
-        }
-        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 14);     // merge + z stores issued
-        if (kCand && pass_a) {
-            __syncwarp();
-            float val[4]; uint32_t src;
-            chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
-            if ((ca[o].kind & 1) && chunk_ok && part == 0) {
-                const size_t chunk = (static_cast<size_t>(row_base + 2 * o) * NT + nb) >> 5;
-                *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
-                p.cand_src[chunk] = src;
-            }
-            __syncwarp();
-        }
-        if (pass_b) {                                             // slots of two unpaired rows: the request at the odd row
-            char* zq = zp + NT * sizeof(float);
-            asm volatile("" : "+l"(zq));
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const SlotCoefB t = cb[j];
-                const float a1 = __uint_as_float(v[2 * j + 1]);
-                const float z1 = fmaf(t.c11, a1, bias * t.d1);
-                const bool own = (c[j].kind & 2) != 0;
-                st_global_f32_if(zq, z1, own && spill);
-                zq += row_stride;
-                if (kTap && own && n_ok) tp[static_cast<size_t>(2 * j + 1) * NT] = a1 + bias;
-                if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z1 + 0.0f : -INFINITY;
-            }
-            if (kCand) {
-                __syncwarp();
-                float val[4]; uint32_t src;
-                chunk_top4_two_lanes(stg + o * kStgPitch, part, val, src);
-                if ((ca[o].kind & 2) && chunk_ok && part == 0) {
-                    const size_t chunk = (static_cast<size_t>(row_base + 2 * o + 1) * NT + nb) >> 5;
-                    *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
-                    p.cand_src[chunk] = src;
-                }
-                __syncwarp();
-            }
-        }
+        finish_slab<kTap, kCand>(p, v, c, ca, cb, stg, row_base, n, nb, n_ok, chunk_ok, bias, lane, !narrow || half == 0,
+                                 !narrow || half == 1);
         if (warp == kCtrlWarps && lane == 0) { CFGMS_TRACE_MARK(p.trace, 8); CFGMS_TRACE_MARK(p.trace, 9); }
     } else {
-        // ================= epilogue (warps 3..10, every CTA) =================
-        // batch parameters are read and z / candidates / counters written from here on
+        // ================= epilogue, slab form (warps 3 .. 3 + EW - 1, every CTA) =================
+        // EW / 4 warps per TMEM lane quarter walk the tile's 32-column slabs; every slab goes through finish_slab (the
+        // branch-free form written for the split-K epilogue): 13 k instead of 20 k cycles per 192-row tile of config 4.
+        // (Twelve or sixteen epilogue warps at 128 / 96 registers measured no faster / slower than eight at 146.)
         pdl_wait_primary();
-        // Let the finalize grid (K2, launched with programmatic stream serialization) be scheduled beside
-        // this one: it consumes finished (stream, row block) groups through p.ready while the GEMM is still
-        // running.  Only after the wait above: K2 of THIS step must not poll the ready counters before K2
-        // of the previous step has re-armed them.  (Transitive ordering is assumed here, as everywhere a kernel
-        // chains programmatic launches: K2's inputs from the PREVIOUS step's K2 — the delay ring, the
-        // device-resident request state — are visible to it because this thread saw that grid complete before
-        // it allowed K2 to start; K2 reads them through L2 (ld.cg), never through a possibly stale L1 line.)
         pdl_launch_dependents();
         const int ew = warp - kCtrlWarps;
-        const int quarter = warp & 3;             // TMEM lane quarter this warp may read
-        const int half = ew >> 2;                 // which slab pairs (alternating) this warp takes
-        const int et = ew * 32 + lane;            // 0..255 among epilogue threads
-        float* stg = reinterpret_cast<float*>(smem_gen + (smem_stg - smem_base)) + ew * (32 * kStgPitch);
-        const int nsp = BN / 64;                  // 64-column slab pairs per tile
+        const int quarter = warp & 3;
+        const int sub = ew >> 2;                  // which of the quarter's EW / 4 warps
+        constexpr int WPQ = EW / 4;
+        const int et = ew * 32 + lane;
+        float* stg = reinterpret_cast<float*>(smem_gen + (smem_stg - smem_base)) + ew * (16 * kStgPitch);
+        const int n_slab = BN / 32;
         const int slots_per_rb = BN / 2;
-        const bool full_table = p.num_row_blocks * slots_per_rb <= kCoefSlots;
         const uint32_t tempty_sig = (kPair && !leader) ? mapa_shared(bar_tempty, leader_rank) : bar_tempty;
-        const size_t NT = static_cast<size_t>(p.NT);
+        const bool full_table = p.num_row_blocks * slots_per_rb <= kCoefSlots;
         if (full_table) {
             // coefficients of every slot, once (the first mainloop hides it)
-            for (int slot = et; slot < p.num_row_blocks * slots_per_rb; slot += 32 * kEpiWarps) {
+            for (int slot = et; slot < p.num_row_blocks * slots_per_rb; slot += 32 * EW) {
                 SlotCoefA ca; SlotCoefB cb;
                 make_slot_coef(p, p.row0 + 2 * slot, ca, cb);
                 coef_a[slot] = ca; coef_b[slot] = cb;
             }
-            named_bar_sync(1, 32 * kEpiWarps);
+            named_bar_sync(1, 32 * EW);
         }
         int acc = 0;
         uint32_t acc_phase = 0;
@@ -556,138 +545,55 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             const int rb = tile % p.num_row_blocks;
             const int vp = tile / p.num_row_blocks;
             const int vt = kPair ? vp * 2 + static_cast<int>(cta_rank) : vp;
-            if (!full_table && rb != cur_rb) {
-                named_bar_sync(1, 32 * kEpiWarps);    // everyone finished reading the old table
+            if (!full_table && rb != cur_rb) {            // more than 1024 rows: the table holds one row block at a time
+                named_bar_sync(1, 32 * EW);               // everyone finished reading the old table
                 if (et < slots_per_rb) {
                     SlotCoefA ca; SlotCoefB cb;
                     make_slot_coef(p, p.row0 + rb * BN + 2 * et, ca, cb);
                     coef_a[et] = ca; coef_b[et] = cb;
                 }
-                named_bar_sync(1, 32 * kEpiWarps);
+                named_bar_sync(1, 32 * EW);
                 cur_rb = rb;
             }
             const int slot_base = full_table ? rb * slots_per_rb : 0;
             const int nb = vt * kBM + quarter * 32;       // first token of this warp's chunk
             const int n = nb + lane;
             const bool n_ok = n < p.NT;
-            const bool chunk_ok = nb < p.NT;              // NT % 32 == 0 on the candidate path
+            const bool chunk_ok = nb < p.NT;
             const float bias = n_ok ? __ldg(p.bias + n) : 0.f;
-
             mbar_wait(bar_tfull + 8 * acc, acc_phase, p.err, 4);
             tc_fence_after();
             if (warp == kCtrlWarps && lane == 0 && tile == worker) CFGMS_TRACE_MARK(p.trace, 7);      // first accumulator complete
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + acc * BN;
-            if (half >= nsp) {                            // nothing to read for this warp: release at once
+            if (sub >= n_slab) {                          // nothing to read for this warp: release at once
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) { if (kPair && !leader) mbar_arrive_cluster(tempty_sig + 8 * acc); else mbar_arrive(bar_tempty + 8 * acc); }
             }
-            for (int sp = half; sp < nsp; sp += 2) {
-                uint32_t v[64];
-                tmem_ld_32x32b_x32(taddr + sp * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
-                tmem_ld_32x32b_x32(taddr + sp * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
+            for (int sl = sub; sl < n_slab; sl += WPQ) {
+                uint32_t v[32];
+                tmem_ld_32x32b_x32(taddr + sl * 32, v);
+                const SlotCoefA* ca = coef_a + slot_base + sl * 16;
+                const SlotCoefB* cb = coef_b + slot_base + sl * 16;
+                SlotCoefA c[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) c[j] = ca[j];
                 tmem_ld_wait();
-                if (sp + 2 >= nsp) {
-                    // this warp's share of the accumulator stage is in registers: hand it back
+                if (sl + WPQ >= n_slab) {                 // this warp's share of the accumulator stage is in registers
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) { if (kPair && !leader) mbar_arrive_cluster(tempty_sig + 8 * acc); else mbar_arrive(bar_tempty + 8 * acc); }
                 }
-                const int row_base = p.row0 + rb * BN + sp * 64;      // batch row of the slab pair's first column
-                const SlotCoefA* ca = coef_a + slot_base + sp * 32;
-                const SlotCoefB* cb = coef_b + slot_base + sp * 32;
-                float* zp = p.z + static_cast<size_t>(row_base) * NT + n;
-                float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
-                int any_odd = 0;
-                // ---- pass A: the request at the even row of every slot.  Row pointers advance by a
-                // fixed stride so that the stores stay predicated (no per-row address rebuild, no branch).
-                const int own_even = n_ok ? 1 : 0, own_odd = n_ok ? 2 : 0;   // kind bits this thread may act on
-                const size_t row_stride = 2 * NT * sizeof(float);      // bytes between the even rows of two slots
-                const bool spill = !(p.probe & 2);
-                {
-                    char* zq = reinterpret_cast<char*>(zp);
-                    char* tq = reinterpret_cast<char*>(tp);
-                    asm volatile("" : "+l"(zq));      // one running per-thread pointer, not base + offset pairs
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const SlotCoefA c = ca[j];
-                        const float a0 = __uint_as_float(v[2 * j]);
-                        const float a1 = __uint_as_float(v[2 * j + 1]);
-                        const float z0 = fmaf(c.c00, a0, fmaf(c.c01, a1, bias * c.d0));
-                        const bool own = (c.kind & own_even) != 0;
-                        any_odd |= c.kind;
-                        st_global_f32_if(zq, z0, own && spill);       // predicated, no branch: the unrolled loop pipelines
-                        if (kTap) {
-                            if (own) { const SlotCoefB t = cb[j]; *reinterpret_cast<float*>(tq) = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
-                            tq += row_stride;
-                        }
-                        zq += row_stride;
-                        if (kCand) stg[j * kStgPitch + lane] = own ? z0 + 0.0f : -INFINITY;
-                    }
-                }
-                if (kCand && (p.probe & 1)) {
-                    // measurement probe: the noise of every merged logit of the slab pair, drawn here (rolled loop over
-                    // the staged z values so that the product path's code stays as it is)
-                    uint32_t sink = 0u;
-#pragma unroll 1
-                    for (int j = 0; j < 32; ++j)
-                        sink ^= __float_as_uint(stg[j * kStgPitch + lane] +
-                                                gumbel_noise(0x1234u, 0x5678u, static_cast<uint32_t>(row_base + 2 * j), 7, n >> 11, n & 2047));
-                    if (sink == 0x9e3779b9u) *p.probe_sink = sink;    // keeps the draws alive
-                }
-                if (kCand) {
-                    __syncwarp();
-                    if ((ca[lane].kind & 1) && chunk_ok) {
-                        float val[4]; uint32_t src;
-                        chunk_top4(stg + lane * kStgPitch, val, src);
-                        const size_t chunk = (static_cast<size_t>(row_base + 2 * lane) * NT + nb) >> 5;
-                        *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
-                        p.cand_src[chunk] = src;
-                    }
-                    __syncwarp();
-                }
-                // ---- pass B: slots that hold two unpaired rows — the request at the odd row
-                if (any_odd & 2) {
-                    char* zq = reinterpret_cast<char*>(zp + NT);
-                    char* tq = kTap ? reinterpret_cast<char*>(tp + NT) : nullptr;
-                    asm volatile("" : "+l"(zq));
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const int kind = ca[j].kind;
-                        const SlotCoefB c = cb[j];
-                        const float a1 = __uint_as_float(v[2 * j + 1]);
-                        const float z1 = fmaf(c.c11, a1, bias * c.d1);
-                        const bool own = (kind & own_odd) != 0;
-                        st_global_f32_if(zq, z1, own);
-                        if (kTap) {
-                            if (own) *reinterpret_cast<float*>(tq) = a1 + bias;
-                            tq += row_stride;
-                        }
-                        zq += row_stride;
-                        if (kCand) stg[j * kStgPitch + lane] = own ? z1 + 0.0f : -INFINITY;
-                    }
-                    if (kCand) {
-                        __syncwarp();
-                        if ((ca[lane].kind & 2) && chunk_ok) {
-                            float val[4]; uint32_t src;
-                            chunk_top4(stg + lane * kStgPitch, val, src);
-                            const size_t chunk = (static_cast<size_t>(row_base + 2 * lane + 1) * NT + nb) >> 5;
-                            *reinterpret_cast<float4*>(p.cand_val + chunk * 4) = make_float4(val[0], val[1], val[2], val[3]);
-                            p.cand_src[chunk] = src;
-                        }
-                        __syncwarp();
-                    }
-                }
+                finish_slab<kTap, kCand>(p, v, c, ca, cb, stg, p.row0 + rb * BN + sl * 32, n, nb, n_ok, chunk_ok, bias, lane, true, true);
             }
             if (p.ready && vt * kBM < p.NT) {
-                // this warp's z / candidate stores of the tile are issued: publish them (release) to K2
                 __syncwarp();
                 if (lane == 0) red_release_gpu_add(p.ready + ((vt * kBM) / p.V) * p.num_row_blocks + rb, 1);
             }
             if (warp == kCtrlWarps && lane == 0 && tile == worker) CFGMS_TRACE_MARK(p.trace, 8);      // first epilogue done
             if (++acc == 2) { acc = 0; acc_phase ^= 1; }
         }
-        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 9);                            // all epilogues done
+        if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 9);
     }
 
     tc_fence_before();
