@@ -488,7 +488,6 @@ __device__ __forceinline__ void head_gemm_body(const CUtensorMap& tmap_w, const 
             tmem_ld_wait();
         }
         if (warp == kCtrlWarps && lane == 0) CFGMS_TRACE_MARK(p.trace, 12);     // partial sums sent
-        const size_t NT = static_cast<size_t>(p.NT);
         const int row_base = p.row0 + rb * BN + col0;
         const SlotCoefA* ca = coef_a + rb * (BN / 2) + (col0 >> 1);
         const SlotCoefB* cb = coef_b + rb * (BN / 2) + (col0 >> 1);
