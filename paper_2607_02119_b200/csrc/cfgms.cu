@@ -289,7 +289,7 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
             return CFGMS_ERR_CUDA;
         }
     }
-    bool attr_ok = static_cast<int>(GemmSmemLayout::total(kMaxBN, 2)) <= c->max_smem_optin;
+    bool attr_ok = static_cast<int>(GemmSmemLayout::total(kMaxBN, 2, true)) <= c->max_smem_optin;
     auto set_smem = [&](const void* fn) {
         attr_ok = attr_ok && cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem_optin) == cudaSuccess;
     };
@@ -413,7 +413,7 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     gp.num_tiles = (pair ? (gp.num_vocab_tiles + 1) / 2 : gp.num_vocab_tiles) * nrb;   // tiles of one worker (CTA or CTA pair)
     gp.num_kb = (c->d + kBK - 1) / kBK;
     const uint32_t stage_bytes = GemmSmemLayout::a_bytes() + GemmSmemLayout::b_bytes(b_rows);
-    int stages = static_cast<int>((static_cast<uint32_t>(c->max_smem_optin) - 1024 - GemmSmemLayout::misc_bytes()) / stage_bytes);
+    int stages = static_cast<int>((static_cast<uint32_t>(c->max_smem_optin) - 1024 - GemmSmemLayout::misc_bytes(split)) / stage_bytes);
     stages = std::max(2, std::min(stages, std::min(kMaxStages, c->max_stages)));
     gp.stages = stages;
     gp.pair_map = a->pair_map; gp.w = a->w; gp.temp = a->temp; gp.phase = a->phase;
@@ -440,7 +440,7 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
 #ifdef CFGMS_TRACE
     gp.trace = c->trace_k1;
 #endif
-    const size_t smem = GemmSmemLayout::total(b_rows, stages);
+    const size_t smem = GemmSmemLayout::total(b_rows, stages, split);
     gp.row0 = 0;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
     // One launch for the whole batch — or, in host-buffer mode, one launch per uploaded chunk of row blocks: chunk k + 1

@@ -100,10 +100,12 @@ struct GemmSmemLayout {
     __host__ __device__ static constexpr uint32_t a_bytes() { return kBM * kBK * 2; }
     __host__ __device__ static constexpr uint32_t b_bytes(int rows) { return static_cast<uint32_t>(rows) * kBK * 2; }
     __host__ __device__ static constexpr uint32_t coef_bytes() { return kCoefSlots * (sizeof(SlotCoefA) + sizeof(SlotCoefB)); }
-    __host__ __device__ static constexpr uint32_t stg_bytes() { return kEpiWarps * 32 * kStgPitch * 4; }
-    __host__ __device__ static constexpr uint32_t misc_bytes() { return coef_bytes() + 256 + stg_bytes(); }
-    __host__ __device__ static constexpr uint32_t total(int b_rows, int stages) {
-        return 1024 + stages * (a_bytes() + b_bytes(b_rows)) + misc_bytes();
+    // transpose stage: 16 requests x 32 tokens per epilogue warp; the split-K build also receives its partner's 4 KB of
+    // partial sums there, so it keeps 32 rows
+    __host__ __device__ static constexpr uint32_t stg_bytes(bool split) { return kEpiWarps * (split ? 32 : 16) * kStgPitch * 4; }
+    __host__ __device__ static constexpr uint32_t misc_bytes(bool split) { return coef_bytes() + 256 + stg_bytes(split); }
+    __host__ __device__ static constexpr uint32_t total(int b_rows, int stages, bool split) {
+        return 1024 + stages * (a_bytes() + b_bytes(b_rows)) + misc_bytes(split);
     }
 };
 
