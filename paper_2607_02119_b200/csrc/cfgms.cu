@@ -440,7 +440,17 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
 #ifdef CFGMS_TRACE
     gp.trace = c->trace_k1;
 #endif
-    const size_t smem = GemmSmemLayout::total(b_rows, stages, split);
+    size_t smem = GemmSmemLayout::total(b_rows, stages, split);
+    if (overlap) {
+        // The finalize kernel's CTAs must become resident BESIDE this kernel: cap the ring so that one of them fits, and ask
+        // for the whole remainder — a smaller request lets the driver pick a smaller shared-memory carve-out for the SM
+        // (196 KiB instead of 228), which leaves the finalize CTA no room at all (cfgms_overlap_stats then reads 0).
+        const size_t k2_need = static_cast<size_t>(kCandWarps) * cand_warp_words(c->V) * 4 + 2048;
+        const size_t budget = static_cast<size_t>(c->max_smem_optin) - k2_need;
+        while (stages > 2 && GemmSmemLayout::total(b_rows, stages, split) > budget) --stages;
+        gp.stages = stages;
+        smem = std::max<size_t>(GemmSmemLayout::total(b_rows, stages, split), budget);
+    }
     gp.row0 = 0;
     if (prof) cudaEventRecord(c->prof_ev[3 * c->prof_n + 0], st);
     // One launch for the whole batch — or, in host-buffer mode, one launch per uploaded chunk of row blocks: chunk k + 1

@@ -375,6 +375,22 @@ def test_overlapped_finalize_equals_serial_finalize(dev):
     ov.check_no_device_error()
 
 
+def test_finalize_really_runs_beside_the_large_gemm(dev):
+    """Config 5 in the default policy: the finalize kernel must be RESIDENT beside the head GEMM, i.e. a good share of its
+    cells reach their readiness check before the GEMM has finished their group.  (Regression: a head GEMM that asks for
+    less shared memory lets the driver pick a smaller carve-out, the finalize CTAs no longer fit, everything still
+    computes the same tokens — and the overlap silently turns into a serial launch.)"""
+    wl = workloads.make_config(5)
+    dw = DeviceWorkload(wl, dev)
+    for t in (16, 17, 18):
+        dw.step(t)
+    torch.cuda.synchronize()
+    assert dw.ctx.info()["overlap"] == 1
+    waited = dw.ctx.overlap_stats()
+    assert waited >= 3 * wl.n_req * wl.S // 4, f"only {waited} of {3 * wl.n_req * wl.S} cells met a running GEMM"
+    dw.check_no_device_error()
+
+
 def test_overlap_counters_survive_steps_whose_cells_are_mostly_pad(dev):
     """Regression: at tau = 0 only stream 0 samples; if PAD cells did not wait for their group the
     finalize grid could finish (and re-arm the ready counters) while the GEMM was still signalling,
