@@ -53,6 +53,7 @@ struct cfgms_ctx {
     int poll_ns = 2000;       // K2's sleep between polls of a ready counter: 1-4 us measured ~2.4 % faster than 50-200 ns at config 5
     int pair_mode = 0;                // 0 = chosen per step, 1 = never pair CTAs, 2 = always pair
     int split_mode = 0;               // split-K for one-wave GEMMs: 0 = chosen per step, 1 = never
+    int max_clusters4 = 0;            // four-CTA clusters of the split-K kernel that can be co-resident on this device
     bool pdl_finalize = true;         // serial mode: launch a small K2 grid as a programmatic dependent of K1
     int probe = 0;                    // measurement probes (CFGMS_CFG_PROBE_*), see GemmParams::probe
     const __nv_bfloat16* heads = nullptr;
@@ -124,7 +125,7 @@ void choose_row_tile(const cfgms_ctx* c, int R, int* BN, int* nrb, bool* pair, b
     if (c->split_mode != 1 && c->overlap_mode != 2 && c->row_tile_override == 0 && c->pair_mode != 1 && vt >= 2 && c->d >= 8 * kBK) {
         const int rb = (R + 127) / 128;
         const int tiles = ((vt + 1) / 2) * rb;
-        if (rb * 64 <= kCoefSlots && tiles * 4 <= c->num_sms) {
+        if (rb * 64 <= kCoefSlots && tiles * 4 <= c->num_sms && tiles <= c->max_clusters4) {
             *BN = 128; *nrb = rb; *pair = true; *split = true;
             return;
         }
@@ -316,6 +317,19 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     if (!attr_ok) {
         cfgms_destroy(c);
         return CFGMS_ERR_CUDA;
+    }
+    {   // how many four-CTA clusters of the split-K kernel fit at once (GPC shapes decide; 0 disables split-K)
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3(4 * static_cast<unsigned>(c->num_sms / 4));
+        lc.blockDim = dim3(kGemmThreads);
+        lc.dynamicSmemBytes = static_cast<size_t>(c->max_smem_optin);
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 4; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        lc.attrs = at; lc.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, cfgms_head_gemm_splitk_kernel<false, true>, &lc) != cudaSuccess) { n = 0; cudaGetLastError(); }
+        c->max_clusters4 = n;
     }
     if (cudaFuncSetAttribute(cfgms_finalize_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024) != cudaSuccess ||
         (V > 256 * 32 && cudaFuncSetAttribute(cfgms_finalize_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
