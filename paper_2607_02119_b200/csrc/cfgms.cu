@@ -546,6 +546,8 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     fp.stats = overlap ? reinterpret_cast<unsigned long long*>(c->ready + (c->ready_words - 32)) : nullptr;
     fp.err = c->err;
     fp.BN = BN; fp.num_row_blocks = nrb;
+    fp.magic_per_stream = fast_div_magic(2 * ((a->R + 1) / 2));
+    fp.magic_bn = fast_div_magic(BN);
     fp.stream_base = c->stream_base; fp.stream_stride = c->stream_stride;
     fp.S_total = c->S_total > 0 ? c->S_total : c->S;
     fp.phase = a->phase; fp.phase_pos = a->phase_pos;

@@ -62,6 +62,9 @@ struct FinalizeParams {
     unsigned long long* stats;// [16] cells that arrived before their group was complete (summed on the host)
     int* err;                 // sticky error word
     int BN, num_row_blocks, ready_target;
+    // host-computed reciprocals (fast_div): x / d == (x * magic) >> 40 exactly for x * d < 2^40
+    unsigned long long magic_per_stream;   // d = 2 * ceil(R / 2): cells per stream
+    unsigned long long magic_bn;           // d = BN
     int poll_ns;              // sleep between two polls of a ready counter
     int pdl_wait;             // 1: launched as a programmatic dependent of K1 WITHOUT ready counters: the per-request
                               //    parameters are fetched while K1 still runs, then griddepcontrol.wait orders
@@ -92,6 +95,13 @@ struct FinalizeParams {
     unsigned long long* trace;
 #endif
 };
+
+// x / d for small non-negative x with magic = ceil(2^40 / d) (host: fast_div_magic): one wide multiply and a shift
+// instead of the ~30-instruction division by a run-time value every cell would otherwise start with.
+__host__ __device__ inline unsigned long long fast_div_magic(int d) { return ((1ull << 40) + static_cast<unsigned>(d) - 1) / static_cast<unsigned>(d); }
+__device__ __forceinline__ int fast_div(int x, unsigned long long magic) {
+    return static_cast<int>((static_cast<unsigned long long>(static_cast<unsigned>(x)) * magic) >> 40);
+}
 
 // Philox4x32-10 (Salmon et al. 2011): ten rounds of two 32x32->64 multiplies with key bumps.
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
@@ -210,7 +220,8 @@ __device__ __forceinline__ void write_cell(const FinalizeParams& p, int r, int i
         __threadfence_system();        // ordered before this CTA's arrival below
     }
     if (p.delayed && audio) {          // only audio-phase tokens belong to the codebook matrix
-        const int slot = ((tau % p.T_cap) + p.T_cap) % p.T_cap;
+        // ring slot tau mod T_cap (non-negative); a ring as deep as the request's lifetime needs no division at all
+        const int slot = (tau >= 0 && tau < p.T_cap) ? tau : ((tau % p.T_cap) + p.T_cap) % p.T_cap;
         p.delayed[(static_cast<size_t>(r) * p.T_cap + slot) * p.S + i] = token;
     }
     if (global_stream(p, i) == 0) {
@@ -644,7 +655,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
     const int per_stream = 2 * slots;
     const int cell = blockIdx.x * kCandWarps + warp;
     const bool in_grid = cell < per_stream * p.S;
-    const int i = in_grid ? cell / per_stream : 0;
+    const int i = in_grid ? fast_div(cell, p.magic_per_stream) : 0;
     const int rem = in_grid ? cell - i * per_stream : 0;
     const int half = rem >= slots ? 1 : 0;
     const int r_raw = 2 * (rem - half * slots) + half;
@@ -691,7 +702,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
         // epilogue warps' red.release.  EVERY request-owning cell waits, also a PAD or forced one that
         // reads nothing: the last CTA of this grid re-arms the counters, which is only safe once
         // every group is complete, i.e. once K1 will not signal again.  Bounded: a pipeline bug fails loudly.
-        const int* flag = p.ready + i * p.num_row_blocks + r / p.BN;
+        const int* flag = p.ready + i * p.num_row_blocks + fast_div(r, p.magic_bn);
         if (lane == 0 && ld_acquire_gpu(flag) < p.ready_target) {
             atomicAdd(p.stats + (blockIdx.x & 15), 1ull);   // evidence counter, spread over 16 words
             const uint64_t t0 = global_timer_ns();
