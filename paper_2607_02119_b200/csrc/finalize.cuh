@@ -810,13 +810,26 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                 m_in = __shfl_sync(0xffffffffu, m_in, owner);
                 uint32_t tE = 0u;
                 if (m_in <= 32) {
-                    // rank the few values of that bucket exactly
+                    // rank the few values of that bucket exactly: every lane counts its members, one warp scan gives
+                    // each lane its place in small[] (no atomics with a return value on the latency chain)
+                    int mine_b = 0;
 #pragma unroll
                     for (int j = 0; j < CPL; ++j)
 #pragma unroll
                         for (int e = 0; e < 4; ++e)
-                            if (key[j][e] >= lo && static_cast<int>((key[j][e] - lo) >> shift) == bucket)
-                                small[atomicAdd(&misc[0], 1)] = key[j][e];
+                            mine_b += (key[j][e] >= lo && static_cast<int>((key[j][e] - lo) >> shift) == bucket) ? 1 : 0;
+                    int at = mine_b;
+#pragma unroll
+                    for (int off = 1; off < 32; off <<= 1) {
+                        const int t = __shfl_up_sync(0xffffffffu, at, off);
+                        if (lane >= off) at += t;
+                    }
+                    at -= mine_b;
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (key[j][e] >= lo && static_cast<int>((key[j][e] - lo) >> shift) == bucket) small[at++] = key[j][e];
                     __syncwarp();
                     const uint32_t x = lane < m_in ? small[lane] : 0u;
                     int gt = 0, ge = 0;
@@ -841,23 +854,41 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
                 }
                 CFGMS_K2_MARK(4);  // t_E known
                 // ---- candidate list {z >= t_E}; overflowing chunks are re-read in full
+                // (every lane counts its entries, one warp scan places them: one shuffle chain instead of a ballot per value)
                 int n_list = 0;
                 uint32_t any_overflow = 0u;
+                {
+                    int mine_l = 0;
+                    bool my_ovf = false;
 #pragma unroll
-                for (int j = 0; j < CPL; ++j) {
-                    const int c = j * 32 + lane;
-                    const bool ovf = c < G && (key[j][3] | 31u) >= tE;
-                    any_overflow |= __ballot_sync(0xffffffffu, ovf);
+                    for (int j = 0; j < CPL; ++j) {
+                        const int c = j * 32 + lane;
+                        const bool ovf = c < G && (key[j][3] | 31u) >= tE;
+                        my_ovf |= ovf;
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const bool pred = c < G && !ovf && key[j][e] >= tE;
-                        const uint32_t b = __ballot_sync(0xffffffffu, pred);
-                        if (pred) {
-                            const int pos = n_list + __popc(b & ((1u << lane) - 1u));
-                            list_key[pos] = key[j][e];
-                            list_v[pos] = tok0 + c * 32 + static_cast<int>((src[j] >> (8 * e)) & 31u);
+                        for (int e = 0; e < 4; ++e) mine_l += (c < G && !ovf && key[j][e] >= tE) ? 1 : 0;
+                    }
+                    any_overflow = __ballot_sync(0xffffffffu, my_ovf);
+                    int at = mine_l;
+#pragma unroll
+                    for (int off = 1; off < 32; off <<= 1) {
+                        const int t = __shfl_up_sync(0xffffffffu, at, off);
+                        if (lane >= off) at += t;
+                    }
+                    n_list = __shfl_sync(0xffffffffu, at, 31);
+                    at -= mine_l;
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j) {
+                        const int c = j * 32 + lane;
+                        const bool ovf = c < G && (key[j][3] | 31u) >= tE;
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            if (c < G && !ovf && key[j][e] >= tE) {
+                                list_key[at] = key[j][e];
+                                list_v[at] = tok0 + c * 32 + static_cast<int>((src[j] >> (8 * e)) & 31u);
+                                ++at;
+                            }
                         }
-                        n_list += __popc(b);
                     }
                 }
                 uint32_t thr = tE;
