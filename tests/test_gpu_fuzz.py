@@ -1,4 +1,4 @@
-"""Seeded randomized parity sweep (160 cases): random shapes and per-request sampler parameters, with and
+"""Seeded randomized parity sweep (200 cases; the last 40 with d >= 512, where one-wave shapes run as split-K clusters): random shapes and per-request sampler parameters, with and
 without vocabulary masks, forced tokens, drain and ring buffers, against the oracle through the C
 ABI.  Small sizes (the oracle computes every cell), but shapes are drawn to hit every kernel path:
 V % 32 != 0 and V % 128 != 0 (full-scan sampler, no overlap), K tails (d % 64 != 0), ragged last
@@ -20,6 +20,8 @@ def _case(seed):
     S = int(rng.integers(1, 11))
     V = int(rng.choice([16, 40, 96, 128, 160, 256, 320, 384, 520, 1024]))
     d = int(rng.choice([64, 72, 128, 200, 256, 320]))
+    if seed >= 160:      # deep enough for the split-K clusters (d >= 512; one-wave shapes take them by default)
+        d = int(rng.choice([512, 584, 640, 768]))
     pairs = int(rng.integers(0, 40))
     singles = 2 * int(rng.integers(0 if pairs else 1, 12))
     T = int(rng.integers(S + 2, S + 14))
@@ -62,7 +64,7 @@ def _case(seed):
     return wl, n_frames, bias, force, knobs
 
 
-@pytest.mark.parametrize("seed", range(160))
+@pytest.mark.parametrize("seed", range(200))
 def test_random_configuration_matches_the_oracle(seed):
     dev = torch.device("cuda:0")
     wl, n_frames, bias, force, knobs = _case(seed)
