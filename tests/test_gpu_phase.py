@@ -25,11 +25,12 @@ def _custom(pairs, singles, d, S, V, T=16, mixed=True, **kw):
     dict(V=512, V_text=192, no_candidates=False, bridge=[500, 3, 260], eos=300),     # candidate sampler (V % 32 == 0)
     dict(V=512, V_text=192, no_candidates=True, bridge=[7], eos=300),                # block-per-cell sampler
     dict(V=200, V_text=70, no_candidates=False, bridge=[], eos=150),                 # V % 32 != 0: any region; no bridging
+    dict(V=512, V_text=192, no_candidates=False, bridge=[9, 400], eos=300, d=512),   # deep enough for the split-K head GEMM
 ])
 def test_mixed_batch_through_all_phases(case):
     dev = torch.device("cuda:0")
     V, V_text, bridge, EOS = case["V"], case["V_text"], case["bridge"], case["eos"]
-    wl = _custom(pairs=6, singles=4, d=256, S=4, V=V, T=64)
+    wl = _custom(pairs=6, singles=4, d=case.get("d", 256), S=4, V=V, T=64)
     R, S = wl.R, wl.S
     heads = wl.head_rows()
     pm = wl.pair_map.numpy()
