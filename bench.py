@@ -310,7 +310,7 @@ class Runner:
         us = max(1e3 * (replay_ms(graph_of(True)) - replay_ms(graph_of(False))) / K, 1e-3)
         return us, 4.0 * wl.R * (wl.T + (wl.T - wl.S + 1)) * wl.S
 
-    def time_widenings(self, K: int):
+    def time_widenings(self, K: int, flush=None):
         """Widening kernels at this config: feedback gather-sum alone (CUDA
         events, tables larger than L2), and the step with streaming frame emission switched on."""
         torch = self.torch
@@ -349,8 +349,42 @@ class Runner:
         e1.record()
         torch.cuda.synchronize()
         with_frames = e0.elapsed_time(e1) * 1e3 / K
+        # the same kernel alone, cold, inside a CUDA graph: K x (256 MiB L2 flush + feedback) minus K x flush (no launch overhead)
+        fb_cold_us = None
+        if flush is not None:
+            def graph_of(with_fb: bool):
+                g2 = torch.cuda.CUDAGraph()
+                s2 = torch.cuda.Stream(device=self.dev)
+                s2.wait_stream(torch.cuda.current_stream())
+                with torch.cuda.stream(s2):
+                    flush.add_(1)
+                    self.ctx.feedback(self.tokens, emb, x)
+                torch.cuda.current_stream().wait_stream(s2)
+                torch.cuda.synchronize()
+                with torch.cuda.graph(g2, stream=s2):
+                    for _ in range(20):
+                        flush.add_(1)
+                        if with_fb:
+                            self.ctx.feedback(self.tokens, emb, x)
+                return g2
+
+            def replay_ms(g2):
+                g2.replay()
+                torch.cuda.synchronize()
+                best = None
+                for _ in range(3):
+                    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a0.record()
+                    g2.replay()
+                    a1.record()
+                    torch.cuda.synchronize()
+                    best = a0.elapsed_time(a1) if best is None else min(best, a0.elapsed_time(a1))
+                return best
+            fb_cold_us = max(1e3 * (replay_ms(graph_of(True)) - replay_ms(graph_of(False))) / 20, 1e-3)
         del emb
         return {"feedback_us": fb_us, "feedback_algorithmic_bytes": fb_bytes, "feedback_gbs": fb_bytes / fb_us / 1e3,
+                "feedback_us_cold_in_graph": fb_cold_us,
+                "feedback_gbs_cold_in_graph": (fb_bytes / fb_cold_us / 1e3) if fb_cold_us else None,
                 "step_us_eager": alone, "step_with_frame_emission_us_eager": with_frames}
 
     def time_e2e(self, K: int, warmup: int):
@@ -606,10 +640,12 @@ def main():
         cb, _, _ = oracle_sample(wl)
         line["cpu_baseline"] = cb
         if not args.no_extras and not sharded:
-            wd = main_r.time_widenings(50)
-            wd["feedback_frac_of_hbm_peak"] = wd["feedback_gbs"] / peaks["hbm_gbs"]
-            line["widenings"] = wd
             flush = torch.zeros(256 * 2 ** 20 // 4, dtype=torch.int32, device=dev)
+            wd = main_r.time_widenings(50, flush)
+            wd["feedback_frac_of_hbm_peak"] = wd["feedback_gbs"] / peaks["hbm_gbs"]
+            if wd["feedback_gbs_cold_in_graph"]:
+                wd["feedback_frac_of_hbm_peak_cold_in_graph"] = wd["feedback_gbs_cold_in_graph"] / peaks["hbm_gbs"]
+            line["widenings"] = wd
             k3_us, k3_bytes = main_r.time_deinterleave(flush)
             line["deinterleave"] = {"kernel": "cfgms_deinterleave_kernel", "us_cold_l2": k3_us, "algorithmic_bytes": k3_bytes,
                                     "gbs": k3_bytes / k3_us / 1e3, "frac_of_hbm_peak": k3_bytes / k3_us / 1e3 / peaks["hbm_gbs"],
