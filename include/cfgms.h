@@ -44,7 +44,9 @@ typedef enum {
     CFGMS_ERR_CUDA = 4,   /* a CUDA runtime / driver call failed                               */
     CFGMS_ERR_ARCH = 5,   /* device is not compute capability 10.x                             */
     CFGMS_ERR_NOMEM = 6,
-    CFGMS_ERR_TIMEOUT = 7 /* a device-side pipeline wait gave up (reported asynchronously)     */
+    CFGMS_ERR_TIMEOUT = 7, /* a device-side pipeline wait gave up (reported asynchronously)    */
+    CFGMS_ERR_LIMIT = 8   /* the request needs more than the fixed scratch of an entry point that
+                             never allocates (cfgms_deinterleave_host_static)                  */
 } cfgms_status;
 
 typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
@@ -303,6 +305,49 @@ int cfgms_deinterleave(cfgms_ctx* ctx, const int32_t* delayed, int32_t n, int32_
 /* Same with HOST buffers (copies in, runs, copies out, synchronises). */
 int cfgms_deinterleave_host(cfgms_ctx* ctx, const int32_t* delayed, int32_t n, int32_t T, int32_t S,
                             int32_t* grid_out, void* cuda_stream);
+
+/*
+ * cfgms_deinterleave_host_static — cfgms_deinterleave_host for callers that must not allocate device memory
+ * (same operation: grid[q][f][i] = delayed[q][f + i][i], 0 <= f < T - S + 1).
+ *
+ * Who needs it.  cfgms_create and cfgms_deinterleave_host call cudaMalloc (the latter whenever a batch is larger
+ * than any it has seen).  That is not an option for every host program:
+ *   - a serving engine of the kind the paper builds on hands almost all free HBM to its own cache pool at
+ *     start-up; a cudaMalloc made later, when a request finishes and its codes have to be de-interleaved, can
+ *     simply fail with out-of-memory although the work needs a few MiB;
+ *   - cudaMalloc and cudaFree may synchronise the whole device, so a call made from the decode loop stalls every
+ *     stream that is in flight, not only the caller's;
+ *   - some deployments audit a fixed device-memory budget and forbid allocation after initialisation.
+ * This entry point therefore takes NO context and calls no cudaMalloc, cudaFree, cudaMallocHost or any other
+ * allocating routine, at set-up or later.  Its device staging (the uploaded delayed buffer and the grid before it
+ * is copied back) lives in one array of CFGMS_STATIC_SCRATCH_BYTES that is part of the library image: every GPU
+ * on which this process uses libcfgms.so holds those bytes from the moment the library's device code is loaded
+ * there until the process exits, whether or not this function is ever called.
+ *
+ *   delayed  : HOST int32 [n][T][S]            grid_out : HOST int32 [n][T - S + 1][S]
+ *   (pageable or pinned; only read / written during the call).  Requires T >= S >= 1, S <= 64, n <= 65535;
+ *   n == 0 is a no-op.  Copies in on `cuda_stream`, runs the de-interleave kernel there, copies out and
+ *   synchronises the stream before returning, like cfgms_deinterleave_host.
+ *
+ * Limit: round_up(n*T*S*4, 256) + n*(T-S+1)*S*4 <= CFGMS_STATIC_SCRATCH_BYTES (8 MiB: e.g. 64 requests of 1024
+ * steps x 16 streams).  A larger request is refused with CFGMS_ERR_LIMIT before anything is copied or launched
+ * and grid_out is left untouched; split the batch over several calls (requests are independent).
+ *
+ * First call on a device: the function looks up the array's device address (cudaGetSymbolAddress), checks that
+ * the device is compute capability 10.x and raises the kernel's shared-memory limit.  This happens once per
+ * device, on the calling thread, with that device current; make that first call during start-up, before any
+ * stream capture is begun.  Later calls on the device do none of this.
+ *
+ * Sharing: all calls on one device use the SAME array and it keeps whatever the previous call left there.
+ * Nothing in it has to start at zero — a call overwrites every word it later reads — so no clearing is done.
+ * Two calls whose device work can overlap (different streams, or different threads) race on the array and
+ * return garbage grids: order them yourself.  Calls from one thread are safe because each one returns only
+ * after its stream has drained.
+ * Errors: ARG, SHAPE, LIMIT, ARCH, CUDA (including "no device").
+ */
+#define CFGMS_STATIC_SCRATCH_BYTES (8u << 20)
+int cfgms_deinterleave_host_static(const int32_t* delayed, int32_t n, int32_t T, int32_t S, int32_t* grid_out,
+                                   void* cuda_stream);
 
 /*
  * cfgms_last_device_error — reads the sticky device error word (one small D2H copy that

@@ -26,14 +26,16 @@ CFGMS_CFG_PROBE_NO_SPILL = 512
 CFGMS_FRAMES_UNSET = 2 ** 31 - 1
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
-          5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT"}
+          5: "CFGMS_ERR_ARCH", 6: "CFGMS_ERR_NOMEM", 7: "CFGMS_ERR_TIMEOUT", 8: "CFGMS_ERR_LIMIT"}
+CFGMS_ERR_LIMIT = 8
+CFGMS_STATIC_SCRATCH_BYTES = 8 << 20
 
 EXPORTS = ["cfgms_create", "cfgms_destroy", "cfgms_step", "cfgms_step_host", "cfgms_deinterleave",
            "cfgms_deinterleave_host", "cfgms_last_device_error", "cfgms_get_info", "cfgms_strerror",
            "cfgms_version", "cfgms_profile_enable", "cfgms_profile_read", "cfgms_overlap_stats",
            "cfgms_set_logit_bias", "cfgms_feedback", "cfgms_set_phase_table", "cfgms_exchange_create",
            "cfgms_exchange_connect", "cfgms_exchange_connect_ipc", "cfgms_exchange_wait", "cfgms_exchange_tokens",
-           "cfgms_set_stream_vocab_sizes"]
+           "cfgms_set_stream_vocab_sizes", "cfgms_deinterleave_host_static"]
 
 
 class CfgmsError(RuntimeError):
@@ -93,6 +95,8 @@ def _lib():
             f = getattr(L, name)
             f.restype = C.c_int
             f.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+        L.cfgms_deinterleave_host_static.restype = C.c_int
+        L.cfgms_deinterleave_host_static.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.cfgms_last_device_error.restype = C.c_int
         L.cfgms_last_device_error.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
         L.cfgms_get_info.restype = C.c_int
@@ -159,6 +163,28 @@ def _check(t: Optional[torch.Tensor], name: str, dtype, device_type: str, numel:
         raise ValueError(f"{name} must be contiguous")
     if numel is not None and t.numel() < numel:
         raise ValueError(f"{name}: needs at least {numel} elements, has {t.numel()}")
+
+
+def deinterleave_host_static(delayed: torch.Tensor, grid_out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """cfgms_deinterleave_host_static: CPU int32 [n][T][S] -> CPU int32 [n][T-S+1][S] without a Context and
+    without any device allocation by the library — for processes that cannot call cudaMalloc once they are
+    serving (all free HBM already belongs to the engine's cache pool, or an allocation's device-wide
+    synchronisation would stall the decode streams).  The staging is a fixed CFGMS_STATIC_SCRATCH_BYTES array
+    inside the library: a larger request raises CfgmsError with status CFGMS_ERR_LIMIT (split the batch); calls
+    share that array, so do not run two of them concurrently on one GPU.  Make the first call on a device at
+    start-up (it does a one-time address lookup).  `grid_out` is allocated here on the HOST when not given."""
+    _check(delayed, "delayed", torch.int32, "cpu")
+    if delayed.dim() != 3:
+        raise ValueError("delayed must be [n][T][S]")
+    n, T, S = (int(x) for x in delayed.shape)
+    if grid_out is None:
+        grid_out = torch.empty((n, max(T - S + 1, 0), S), dtype=torch.int32)
+    _check(grid_out, "grid_out", torch.int32, "cpu", n * max(T - S + 1, 0) * S)
+    sp = stream.cuda_stream if stream is not None else (torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0)
+    rc = _lib().cfgms_deinterleave_host_static(delayed.data_ptr(), n, T, S, grid_out.data_ptr(), sp)
+    if rc != 0:
+        raise CfgmsError(rc, "cfgms_deinterleave_host_static")
+    return grid_out
 
 
 class Context:

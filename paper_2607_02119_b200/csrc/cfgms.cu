@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "aux_kernels.cuh"
@@ -191,6 +192,7 @@ const char* cfgms_strerror(int s) {
         case CFGMS_ERR_ARCH: return "device is not sm_100 (no fallback path exists)";
         case CFGMS_ERR_NOMEM: return "out of device memory";
         case CFGMS_ERR_TIMEOUT: return "device-side pipeline wait timed out";
+        case CFGMS_ERR_LIMIT: return "request exceeds the fixed scratch (CFGMS_STATIC_SCRATCH_BYTES) of a non-allocating entry point";
         default: return "unknown status";
     }
 }
@@ -970,3 +972,83 @@ int cfgms_get_info(cfgms_ctx* c, cfgms_info* out) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// cfgms_deinterleave_host_static: the de-interleave with host buffers for callers that must not allocate device
+// memory (a serving engine that gave all free HBM to its cache pool, a decode loop that cannot afford cudaMalloc's
+// device-wide synchronisation, a deployment with a fixed memory budget; include/cfgms.h has the full contract).
+// Nothing below calls cudaMalloc / cudaFree / cudaMallocHost or creates streams or events.
+//
+// The staging the kernel reads from and writes to is this file-scope array.  It is part of the library's device
+// image: each GPU this process runs libcfgms.so on holds these 8 MiB until the process exits.  In HOST code the
+// name g_static_scratch is only a handle for the runtime's symbol table, NOT a device address — handing it to a
+// kernel would make the kernel fault (or, where the GPU can reach host memory, scribble over the host-side shadow).
+// The device address is fetched once per device with cudaGetSymbolAddress and that pointer is what the kernel gets.
+static __device__ __align__(256) unsigned char g_static_scratch[CFGMS_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticScratchDevice {
+    bool ready = false;
+    unsigned char* base = nullptr;     // device address of g_static_scratch on this device
+};
+StaticScratchDevice g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;
+
+// Once per device, with that device current: architecture check, the array's device address, and the shared-memory
+// opt-in the kernel needs from S = 42 on (cfgms_create does the same for contexts; this entry point has none).
+int static_scratch_setup(unsigned char** base_out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CFGMS_ERR_CUDA; }
+    if (dev < 0 || dev >= kStaticMaxDevices) return CFGMS_ERR_ARG;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticScratchDevice& sd = g_static_dev[dev];
+    if (!sd.ready) {
+        int major = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return CFGMS_ERR_CUDA; }
+        if (major != 10) return CFGMS_ERR_ARCH;
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess || !p) { cudaGetLastError(); return CFGMS_ERR_CUDA; }
+        if (cudaFuncSetAttribute(cfgms_deinterleave_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024) != cudaSuccess) {
+            cudaGetLastError();
+            return CFGMS_ERR_CUDA;
+        }
+        sd.base = static_cast<unsigned char*>(p);
+        sd.ready = true;
+    }
+    *base_out = sd.base;
+    return CFGMS_OK;
+}
+
+}  // namespace
+
+extern "C" int cfgms_deinterleave_host_static(const int32_t* delayed, int32_t n, int32_t T, int32_t S, int32_t* grid_out,
+                                              void* cuda_stream) {
+    if (n < 0 || S < 1 || T < S) return CFGMS_ERR_ARG;
+    if (n == 0) return CFGMS_OK;
+    if (!delayed || !grid_out) return CFGMS_ERR_ARG;
+    if (S > 64 || n > 65535) return CFGMS_ERR_SHAPE;
+    const int F = T - S + 1;
+    const size_t in_bytes = static_cast<size_t>(n) * static_cast<size_t>(T) * S * 4;
+    const size_t out_bytes = static_cast<size_t>(n) * static_cast<size_t>(F) * S * 4;
+    const size_t out_off = (in_bytes + 255) & ~static_cast<size_t>(255);      // both halves 256-byte aligned (the kernel needs 16)
+    if (out_off + out_bytes > static_cast<size_t>(CFGMS_STATIC_SCRATCH_BYTES)) return CFGMS_ERR_LIMIT;
+
+    unsigned char* base = nullptr;
+    const int rc = static_scratch_setup(&base);
+    if (rc != CFGMS_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int32_t* d_in = reinterpret_cast<int32_t*>(base);
+    int32_t* d_out = reinterpret_cast<int32_t*>(base + out_off);
+    // The array still holds the previous call's bytes.  That is harmless: the kernel reads d_in[0, n*T*S) only, all of
+    // it uploaded just now, and writes every word of d_out[0, n*F*S), which is all that is copied back.
+    if (cudaMemcpyAsync(d_in, delayed, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return CFGMS_ERR_CUDA; }
+    const dim3 grid((F + kDeintFrames - 1) / kDeintFrames, n);
+    const size_t smem = static_cast<size_t>(kDeintFrames + S - 1) * S * 4;
+    cfgms_deinterleave_kernel<<<grid, kDeintThreads, smem, st>>>(d_in, d_out, T, S);
+    if (cudaGetLastError() != cudaSuccess) { cudaStreamSynchronize(st); return CFGMS_ERR_CUDA; }
+    if (cudaMemcpyAsync(grid_out, d_out, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) { cudaGetLastError(); cudaStreamSynchronize(st); return CFGMS_ERR_CUDA; }
+    if (cudaStreamSynchronize(st) != cudaSuccess) return CFGMS_ERR_CUDA;
+    return CFGMS_OK;
+}
