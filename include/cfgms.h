@@ -100,7 +100,12 @@ typedef struct {
                               means unsharded (base 0, stride 1).  frame_out needs an unsharded context */
     int32_t global_streams; /* stream-sharded heads: the number of streams of the WHOLE head (the drain of a
                                request ends S_global - 1 steps after its last frame); 0 = this context's S.
-                               A sharded context needs it to write step_next_out / n_frames_next_out / done_out */
+                               A sharded context needs it to write step_next_out / n_frames_next_out / done_out.
+                               Only the shard that holds global stream 0 (stream_base == 0) can write the request-state
+                               outputs (step_next_out, n_frames_next_out, done_out, phase_next_out, phase_pos_next_out,
+                               modality_out): the state advances on the primary stream's token.  Any other shard that
+                               asks for them gets CFGMS_ERR_ARG; it takes the next state from the rank with stream 0
+                               (4 small [R] arrays) or keeps passing host-advanced state                         */
 } cfgms_config;
 
 /*
@@ -216,9 +221,11 @@ int cfgms_step(cfgms_ctx* ctx, const cfgms_step_args* args, void* cuda_stream);
 
 /*
  * cfgms_step_host — same step with HOST buffers: hidden, pair_map, w, temp, top_k, step,
- * req_id, n_frames, force_token, tokens_out, frame_out and frame_index_out are HOST pointers
+ * req_id, n_frames, force_token, phase, phase_pos, tokens_out, frame_out and frame_index_out are HOST pointers
  * (pinned memory recommended); `delayed`, `logits_out` and the request-state outputs (`step_next_out`,
- * `n_frames_next_out`, `done_out`) stay DEVICE pointers (per-request state lives in HBM) or NULL.  Copies the
+ * `n_frames_next_out`, `done_out`, `phase_next_out`, `phase_pos_next_out`, `modality_out`) stay DEVICE pointers
+ * (per-request state lives in HBM) or NULL.  Every INPUT of this entry point is a host array, every state OUTPUT a
+ * device array: a caller that keeps the phase state on the device uses cfgms_step.  Copies the
  * inputs host->device, runs the step, copies tokens_out device->host and synchronises the
  * stream.  Bytes moved per call are reported by cfgms_get_info.
  */
@@ -266,13 +273,21 @@ int cfgms_set_stream_vocab_sizes(cfgms_ctx* ctx, const int32_t* sizes, const flo
  *                               mapped by other means; from then on every cfgms_step of this context scatters.
  *   cfgms_exchange_connect_ipc  handles: HOST [world][64] bytes, every rank's IPC handle in rank order; opens the
  *                               peers' blocks (closed at cfgms_destroy) and connects.
- *   cfgms_exchange_wait         enqueues a one-CTA kernel that waits (bounded, 2 s -> CFGMS_ERR_TIMEOUT) until the
+ *   cfgms_exchange_wait         enqueues a one-CTA kernel that waits (bounded, 2 s) until the
  *                               tokens of every rank's current step have landed in this rank's gather buffer, then
  *                               copies rows [0, R) of the step's half to the buffer cfgms_exchange_tokens returns;
  *                               kernels enqueued after it on the stream may read that.  Call it exactly once per
  *                               step.  Epochs are counted on the device: CUDA-graph replay is fine.
  *   cfgms_exchange_tokens       *tokens_all_out = the gathered tokens of the last waited step, DEVICE int32
  *                               [max_rows][S_global] (owned by the context).
+ * A wait that gives up after 2 s latches CFGMS_ERR_TIMEOUT in the sticky error word (cfgms_last_device_error) and
+ * ends the kernel WITHOUT touching the gathered tokens or the step count (the CUDA context stays usable; whatever
+ * the stream runs next reads the previous step's tokens, so check the error word before trusting a step that may
+ * have met a late peer, e.g. the very first one).  A failed cfgms_exchange_create leaves no exchange behind and may
+ * be repeated.  Teardown: peers store into this rank's block until their last step has finished, so synchronise
+ * every rank's stream and pass a barrier of your own (host side) BEFORE any rank calls cfgms_destroy.
+ * Status: the cross-process path (IPC handles, two GPUs) has not yet been run on hardware — no multi-GPU box was
+ * available; the protocol is covered on one GPU (contexts of one process) and by a two-process host model.
  * Errors: ARG (no global stream count, exchange already created / not created), NOMEM, CUDA.
  */
 int cfgms_exchange_create(cfgms_ctx* ctx, int32_t world, int32_t rank, void* ipc_handle_out, void** base_out);

@@ -286,9 +286,10 @@ class Context:
             _check(t, name, torch.int32, "cuda", R, optional=True)
         a.eos_token = int(eos_token)
         a.step_next_out, a.n_frames_next_out, a.done_out = _ptr(step_next_out), _ptr(n_frames_next_out), _ptr(done_out)
-        for t, name in ((phase, "phase"), (phase_pos, "phase_pos"), (phase_next_out, "phase_next_out"),
-                        (phase_pos_next_out, "phase_pos_next_out"), (modality_out, "modality_out")):
-            _check(t, name, torch.int32, "cuda", R, optional=True)
+        for t, name in ((phase, "phase"), (phase_pos, "phase_pos")):          # inputs: where the step's inputs live
+            _check(t, name, torch.int32, dev, R, optional=True)
+        for t, name in ((phase_next_out, "phase_next_out"), (phase_pos_next_out, "phase_pos_next_out"), (modality_out, "modality_out")):
+            _check(t, name, torch.int32, "cuda", R, optional=True)           # request state stays in HBM
         a.phase, a.phase_pos = _ptr(phase), _ptr(phase_pos)
         a.phase_next_out, a.phase_pos_next_out, a.modality_out = _ptr(phase_next_out), _ptr(phase_pos_next_out), _ptr(modality_out)
         return a
@@ -307,10 +308,13 @@ class Context:
 
     def step_host(self, hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id=None, n_frames=None,
                   delayed=None, logits_out=None, stream=None, force_token=None, frame_out=None,
-                  frame_index_out=None) -> None:
-        """cfgms_step_host: host tensors in, host tokens out; synchronises the stream."""
+                  frame_index_out=None, eos_token=-1, step_next_out=None, n_frames_next_out=None, done_out=None,
+                  phase=None, phase_pos=None, phase_next_out=None, phase_pos_next_out=None, modality_out=None) -> None:
+        """cfgms_step_host: host tensors in (phase / phase_pos included), host tokens out; the request-state
+        outputs, `delayed` and `logits_out` are device tensors; synchronises the stream."""
         a = self._args(hidden, pair_map, w, temp, top_k, seed, step, tokens_out, req_id, n_frames, delayed,
-                       logits_out, "cpu", force_token, frame_out, frame_index_out)
+                       logits_out, "cpu", force_token, frame_out, frame_index_out, eos_token, step_next_out,
+                       n_frames_next_out, done_out, phase, phase_pos, phase_next_out, phase_pos_next_out, modality_out)
         rc = _lib().cfgms_step_host(self._h, C.byref(a), _stream_ptr(stream))
         if rc != 0:
             raise CfgmsError(rc, "cfgms_step_host")
@@ -347,7 +351,12 @@ class Context:
         return bytes(handle), int(base.value)
 
     def exchange_connect(self, peer_bases) -> None:
-        """peer_bases: the ranks' block addresses as valid in this process (same-process peers)."""
+        """peer_bases: the ranks' block addresses as valid in this process (same-process peers), one per rank."""
+        world = getattr(self, "_xchg", (None, None))[0]
+        if world is None:
+            raise ValueError("exchange_connect before exchange_create")
+        if len(peer_bases) != world:       # the library reads exactly `world` entries
+            raise ValueError(f"peer_bases needs one entry per rank: world = {world}, got {len(peer_bases)}")
         arr = (C.c_void_p * len(peer_bases))(*[int(b) if b else None for b in peer_bases])
         rc = _lib().cfgms_exchange_connect(self._h, arr)
         if rc != 0:
@@ -358,6 +367,11 @@ class Context:
         blob = b"".join(bytes(h) for h in handles)
         if len(blob) != 64 * len(handles):
             raise ValueError("every handle must be 64 bytes")
+        world = getattr(self, "_xchg", (None, None))[0]
+        if world is None:
+            raise ValueError("exchange_connect_ipc before exchange_create")
+        if len(handles) != world:          # the library reads world x 64 bytes
+            raise ValueError(f"handles needs one entry per rank: world = {world}, got {len(handles)}")
         rc = _lib().cfgms_exchange_connect_ipc(self._h, blob)
         if rc != 0:
             raise CfgmsError(rc, "cfgms_exchange_connect_ipc")

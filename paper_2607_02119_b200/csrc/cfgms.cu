@@ -171,8 +171,14 @@ int validate_step(const cfgms_ctx* c, const cfgms_step_args* a) {
     if ((a->frame_out || a->frame_index_out) && (!a->delayed || a->T_cap < c->S)) return CFGMS_ERR_ARG;
     if ((a->frame_out || a->frame_index_out) && (c->stream_base != 0 || c->stream_stride != 1)) return CFGMS_ERR_ARG;   // a frame needs every stream
     // the drain of a request ends S_global - 1 steps after its last frame: a shard must know S_global
+    const bool state_out = a->step_next_out || a->n_frames_next_out || a->done_out || a->phase_next_out || a->phase_pos_next_out ||
+                           a->modality_out;
     if ((a->step_next_out || a->n_frames_next_out || a->done_out || a->phase_next_out || a->phase_pos_next_out) && c->S_total == 0)
         return CFGMS_ERR_ARG;
+    // The request state advances on what the PRIMARY stream (global stream 0) emitted, by the thread of that cell
+    // (finalize.cuh write_cell).  A shard that does not hold global stream 0 has no such cell: refuse, rather than leave the
+    // outputs silently unwritten and let a device-resident state loop on that rank run on stale state.
+    if (state_out && c->stream_base != 0) return CFGMS_ERR_ARG;
     if (a->phase && (!a->phase_pos || a->force_token)) return CFGMS_ERR_ARG;
     if (!a->phase && (a->phase_pos || a->phase_next_out || a->phase_pos_next_out || a->modality_out)) return CFGMS_ERR_ARG;
     return CFGMS_OK;
@@ -646,8 +652,9 @@ int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     HostStage& h = c->hs;
     const size_t Rmax = static_cast<size_t>(c->max_rows);
     if (!c->hs_ready) {
-        // every per-row input of a step travels in ONE block: seven [R] arrays + force_token [R][S]
-        h.params_bytes = Rmax * 4 * (7 + static_cast<size_t>(c->S));
+        // every per-row input of a step travels in ONE block: nine [R] arrays (the seven of the plain path, phase and
+        // phase_pos) + force_token [R][S]
+        h.params_bytes = Rmax * 4 * (9 + static_cast<size_t>(c->S));
         bool ok = cudaMalloc(&h.hidden, Rmax * c->d * 4) == cudaSuccess &&
                   cudaMalloc(reinterpret_cast<void**>(&h.params), h.params_bytes) == cudaSuccess &&
                   cudaMallocHost(reinterpret_cast<void**>(&h.params_pinned), h.params_bytes) == cudaSuccess &&
@@ -686,6 +693,8 @@ int cfgms_step_host(cfgms_ctx* c, const cfgms_step_args* a, void* cuda_stream) {
     d.req_id = reinterpret_cast<const uint32_t*>(pack(a->req_id, R * 4));
     d.n_frames = reinterpret_cast<const int32_t*>(pack(a->n_frames, R * 4));
     d.force_token = reinterpret_cast<const int32_t*>(pack(a->force_token, R * c->S * 4));
+    d.phase = reinterpret_cast<const int32_t*>(pack(a->phase, R * 4));          // read by the GEMM epilogue and the samplers
+    d.phase_pos = reinterpret_cast<const int32_t*>(pack(a->phase_pos, R * 4));
     if (cudaMemcpyAsync(h.params, h.params_pinned, off, cudaMemcpyHostToDevice, st) != cudaSuccess) return CFGMS_ERR_CUDA;
     h2d += static_cast<int64_t>(off);
     d.tokens_out = h.tokens;
@@ -757,13 +766,15 @@ int cfgms_exchange_create(cfgms_ctx* c, int32_t world, int32_t rank, void* ipc_h
     c->xc.flags_off = 3 * c->xc.half_bytes;
     c->xc.state_off = c->xc.flags_off + 256;
     const size_t total = c->xc.state_off + 256;
-    if (cudaMalloc(&c->xc.base, total) != cudaSuccess) { c->xc.base = nullptr; return CFGMS_ERR_NOMEM; }
-    if (cudaMemset(c->xc.base, 0, total) != cudaSuccess) return CFGMS_ERR_CUDA;
+    if (cudaMalloc(&c->xc.base, total) != cudaSuccess) { c->xc.base = nullptr; cudaGetLastError(); return CFGMS_ERR_NOMEM; }
+    // a failure below leaves no half-made exchange behind: the context is as before the call and may try again
+    auto undo = [&]() { cudaFree(c->xc.base); c->xc.base = nullptr; c->xc.world = 0; c->xc.rank = 0; cudaGetLastError(); return CFGMS_ERR_CUDA; };
+    if (cudaMemset(c->xc.base, 0, total) != cudaSuccess) return undo();
     c->xc.world = world; c->xc.rank = rank;
     if (ipc_handle_out) {
         static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size is part of the ABI");
         cudaIpcMemHandle_t h;
-        if (cudaIpcGetMemHandle(&h, c->xc.base) != cudaSuccess) return CFGMS_ERR_CUDA;
+        if (cudaIpcGetMemHandle(&h, c->xc.base) != cudaSuccess) return undo();
         std::memcpy(ipc_handle_out, &h, sizeof(h));
     }
     if (base_out) *base_out = c->xc.base;
@@ -797,7 +808,21 @@ int cfgms_exchange_connect_ipc(cfgms_ctx* c, const void* handles) {
         if (!c->xc.opened[q]) {
             cudaIpcMemHandle_t h;
             std::memcpy(&h, static_cast<const char*>(handles) + 64 * q, sizeof(h));
+            // fails (ERR_CUDA, nothing connected) when the handle is not a live allocation of another process or the two
+            // devices cannot reach each other: no peer access, no exchange
             if (cudaIpcOpenMemHandle(&c->xc.opened[q], h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+                c->xc.opened[q] = nullptr;
+                cudaGetLastError();
+                return CFGMS_ERR_CUDA;
+            }
+            // lazy peer enabling defers the real check to first use: ask now, so that a pair of GPUs without a peer path
+            // is refused here and not by a faulting store inside the finalize kernel
+            cudaPointerAttributes pa{};
+            int can = 1;
+            if (cudaPointerGetAttributes(&pa, c->xc.opened[q]) == cudaSuccess && pa.device != c->device)
+                if (cudaDeviceCanAccessPeer(&can, c->device, pa.device) != cudaSuccess) { can = 1; cudaGetLastError(); }
+            if (!can) {
+                cudaIpcCloseMemHandle(c->xc.opened[q]);
                 c->xc.opened[q] = nullptr;
                 return CFGMS_ERR_CUDA;
             }

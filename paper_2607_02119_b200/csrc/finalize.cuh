@@ -196,6 +196,10 @@ __device__ __forceinline__ CellPlan plan_cell(const FinalizeParams& p, int r, in
     if (c.hi <= c.lo) c.sample = false;        // empty region: nothing to sample, the cell pads
     return c;
 }
+// TEXT phase with an EMPTY text region (V_text == 0: no phase table installed, or one without text tokens): the cell
+// pads and reads no logits, but the modality inference still has an answer — every token of stream 0 is an audio token,
+// so the unmasked argmax lies in the audio region whatever the logits are (the oracle computes it and gets 1).
+__device__ __forceinline__ int modality_without_logits(const CellPlan& c) { return (c.want_modality && !c.sample) ? 1 : 0; }
 
 // Rows a4 of the hot path, by ONE thread per cell: token to the row and its companion
 // (PAPER.md:93), delayed-layout cell.  The thread of the LAST stream also emits
@@ -322,21 +326,26 @@ __global__ void __launch_bounds__(256)
 cfgms_exchange_wait_kernel(const volatile uint32_t* flags, unsigned int* wait_count, int world, const int32_t* halves,
                            int32_t* latest, int half_elems, int n_copy, int* err) {
     __shared__ unsigned int want;
-    if (threadIdx.x == 0) { want = *wait_count + 1u; }
+    __shared__ int timed_out;
+    if (threadIdx.x == 0) { want = *wait_count + 1u; timed_out = 0; }
     __syncthreads();
     if (static_cast<int>(threadIdx.x) < world) {
         const uint64_t t0 = global_timer_ns();
         while (static_cast<int>(flags[threadIdx.x] - want) < 0) {
             __nanosleep(200);
             if (global_timer_ns() - t0 > 2000000000ull) {
+                // A late peer (first-step module load, a slow rank) must not poison this process's CUDA context: latch the
+                // time-out in the sticky error word and leave.  `latest` and the wait count stay as they were, so the
+                // step can be waited for again once cfgms_last_device_error has reported it.
                 atomicCAS(err, 0, 7 /* CFGMS_ERR_TIMEOUT */ | (11 << 8));
-                __threadfence_system();
-                __trap();
+                timed_out = 1;
+                break;
             }
         }
     }
     __threadfence_system();      // acquire side
     __syncthreads();
+    if (timed_out) return;
     const int32_t* src = halves + static_cast<size_t>(want & 1u) * half_elems;
     for (int e = threadIdx.x; e < n_copy; e += blockDim.x) latest[e] = __ldcv(src + e);
     if (threadIdx.x == 0) *wait_count = want;
@@ -418,7 +427,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_kernel(const Final
     const int tau = cp.gstep;          // keys the noise
     bool active = cp.sample;
     int token = cp.token;
-    int modality = 0;
+    int modality = modality_without_logits(cp);
     if (active) {
         const int ft = forced_token(p, r, i);
         if (ft >= 0) { token = ft; active = false; }
@@ -549,7 +558,7 @@ __global__ void __launch_bounds__(kFinThreads) cfgms_finalize_large_kernel(const
     const int tau = cp.gstep;          // keys the noise
     bool active = cp.sample;
     int token = cp.token;
-    int modality = 0;
+    int modality = modality_without_logits(cp);
     if (active) {
         const int ft = forced_token(p, r, i);
         if (ft >= 0) { token = ft; active = false; }
@@ -695,7 +704,7 @@ __global__ void __launch_bounds__(kCandWarps * 32) cfgms_finalize_cand_kernel(co
 
     bool active = valid && cp.sample;
     int token = cp.token;
-    int modality = 0;
+    int modality = modality_without_logits(cp);
     if (active && ft >= 0) { token = ft; active = false; }
     if (valid && p.ready) {
         // Wait until K1 has written every tile of this (stream, row block): the acquire pairs with the

@@ -173,3 +173,24 @@ def compare_step(dw: DeviceWorkload, t: int, cells, stats: ParityStats, check_lo
     for c in wl.head_rows():
         assert np.array_equal(dl[c, int(tau[c]) % dw.T_cap], got[c])
     return got
+
+
+def check_tokens_against_oracle(wl, t: int, got: np.ndarray) -> int:
+    """A full [R][S] token matrix of step t (e.g. gathered from stream shards) against oracle.step: PAD and
+    every cell outside the oracle's close / boundary flags bit-equal, a differing close cell a valid
+    alternative, companion rows equal to their cond rows.  Returns the number of close cells."""
+    ref = oracle_step(wl, t, want_merged=False)
+    pm = wl.pair_map.numpy()
+    n_close = 0
+    for j, (c, i) in enumerate(ref.cells):
+        fl = int(ref.flags[j])
+        if pm[c] >= 0:
+            assert got[pm[c], i] == got[c, i], (t, c, i)
+        if fl & oracle.FLAG_INACTIVE:
+            assert got[c, i] == wl.pad_token, (t, c, i, got[c, i])
+        elif fl & (oracle.FLAG_CLOSE | oracle.FLAG_BOUNDARY):
+            n_close += 1
+            assert got[c, i] == ref.tok[j] or valid_alternative(wl, t, c, i, int(got[c, i])), (t, c, i, got[c, i], ref.tok[j])
+        else:
+            assert got[c, i] == ref.tok[j], (t, c, i, got[c, i], ref.tok[j], ref.margin[j])
+    return n_close

@@ -158,3 +158,76 @@ def test_phase_arguments_are_validated():
                 n_frames=dw.n_frames, delayed=dw.delayed, phase=torch.full((wl.R,), 2, dtype=torch.int32, device=dev), phase_pos=st)
     torch.cuda.synchronize()
     assert torch.equal(plain, dw.tokens)
+
+
+@pytest.mark.parametrize("no_candidates", [False, True])
+def test_text_phase_with_an_empty_text_region_moves_on(no_candidates):
+    """`phase` passed without a phase table (V_text = 0, no bridging tokens): a TEXT-phase request has nothing to
+    sample, pads — and its unmasked argmax necessarily lies in the audio region, so the modality inference says
+    "audio" and the request enters the audio phase at the next step, exactly as oracle.step_phase /
+    oracle.phase_advance say (it must not sit in TEXT forever)."""
+    dev = torch.device("cuda:0")
+    wl = _custom(pairs=3, singles=2, d=128, S=3, V=160 if no_candidates else 256, T=16)
+    R, S = wl.R, wl.S
+    dw = DeviceWorkload(wl, dev, no_candidates=no_candidates)
+    heads = wl.head_rows()
+    o_phase = np.full(R, PHASE_TEXT, dtype=np.int32)
+    o_pos = np.zeros(R, dtype=np.int32)
+    o_gstep = np.arange(R, dtype=np.int32)
+    o_F = np.full(R, F_UNSET, dtype=np.int32)
+    cu = lambda a: torch.from_numpy(a.copy()).to(dev)
+    out = {k: torch.full((R,), -9, dtype=torch.int32, device=dev) for k in ("phase", "pos", "gstep", "F", "done", "mod")}
+    dw.tokens.fill_(-7)
+    dw.ctx.step(dw.hidden(0), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, cu(o_gstep), dw.tokens, req_id=dw.req_id,
+                n_frames=cu(o_F), delayed=dw.delayed, eos_token=5, step_next_out=out["gstep"], n_frames_next_out=out["F"],
+                done_out=out["done"], phase=cu(o_phase), phase_pos=cu(o_pos), phase_next_out=out["phase"],
+                phase_pos_next_out=out["pos"], modality_out=out["mod"])
+    dw.check_no_device_error()
+    ref = oracle.step_phase(wl.heads, wl.embeds, wl.hidden(0), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, o_gstep,
+                            o_phase, o_pos, 0, [], req_id=wl.req_id, n_frames=o_F, pad_token=wl.pad_token)
+    got = dw.tokens.cpu().numpy()
+    for j, (c, i) in enumerate(ref.cells):
+        assert ref.tok[j] == wl.pad_token and got[c, i] == wl.pad_token
+        if i == 0:
+            assert ref.modality[j] == 1
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    for c in heads:
+        ph, pos, F, d = oracle.phase_advance(PHASE_TEXT, 0, F_UNSET, wl.pad_token, True, 0, 5, S)
+        assert ph == PHASE_AUDIO
+        assert (res["mod"][c], res["phase"][c], res["pos"][c], res["F"][c], bool(res["done"][c])) == (1, ph, pos, F, d), c
+        assert res["gstep"][c] == o_gstep[c] + 1
+
+
+def test_step_host_stages_the_phase_inputs():
+    """cfgms_step_host takes phase / phase_pos as HOST arrays like its other inputs (they travel in the one packed
+    parameter copy); tokens and the device-resident next state equal cfgms_step's on a batch that holds every phase."""
+    dev = torch.device("cuda:0")
+    V, V_text, bridge, EOS = 512, 192, [500, 3], 300
+    wl = _custom(pairs=6, singles=4, d=256, S=4, V=V, T=64)
+    R, S = wl.R, wl.S
+    dw = DeviceWorkload(wl, dev, T_cap=16)
+    dw.ctx.set_phase_table(V_text, bridge)
+    phase = torch.zeros(R, dtype=torch.int32)
+    pos = torch.zeros(R, dtype=torch.int32)
+    for q, c in enumerate(wl.head_rows()):
+        phase[c] = q % 4
+        pos[c] = 1 if q % 4 == PHASE_TRANSITION else (q if q % 4 == PHASE_AUDIO else 0)
+    gstep = torch.arange(R, dtype=torch.int32) + 3
+    names = ("step_next_out", "n_frames_next_out", "done_out", "phase_next_out", "phase_pos_next_out", "modality_out")
+    mk = lambda: {k: torch.full((R,), -9, dtype=torch.int32, device=dev) for k in names}
+    want, have = mk(), mk()
+    dw.tokens.fill_(-7)
+    dw.ctx.step(dw.hidden(2), dw.pair_map, dw.w, dw.temp, dw.top_k, wl.seed, gstep.to(dev), dw.tokens, req_id=dw.req_id,
+                n_frames=dw.n_frames, eos_token=EOS, phase=phase.to(dev), phase_pos=pos.to(dev), **want)
+    dw.check_no_device_error()
+    tok_host = torch.full((R, S), -1, dtype=torch.int32).pin_memory()
+    dw.ctx.step_host(wl.hidden(2).pin_memory(), wl.pair_map, wl.w, wl.temp, wl.top_k, wl.seed, gstep, tok_host,
+                     req_id=wl.req_id, n_frames=wl.n_frames, eos_token=EOS, phase=phase, phase_pos=pos, **have)
+    dw.check_no_device_error()
+    assert torch.equal(tok_host, dw.tokens.cpu())
+    assert len({int(x) for x in phase.numpy()[wl.head_rows()]}) == 4
+    for k in names:
+        assert torch.equal(want[k], have[k]), k
+        assert bool((want[k].cpu().numpy()[wl.head_rows()] != -9).all()), k
+    n_arrays = 5 + 2 + (wl.req_id is not None) + (wl.n_frames is not None)      # the plain path's [R] inputs + phase, phase_pos
+    assert dw.ctx.info()["h2d_bytes_last_step"] == R * wl.d * 2 + n_arrays * R * 4

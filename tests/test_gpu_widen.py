@@ -9,7 +9,7 @@ import torch
 
 import oracle
 import workloads
-from parity_util import LOGIT_TOL, DeviceWorkload
+from parity_util import LOGIT_TOL, DeviceWorkload, check_tokens_against_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -284,6 +284,7 @@ def test_stream_sharded_contexts_sample_what_the_unsharded_head_samples(dev, wor
         torch.cuda.synchronize()
         merged = dist_utils.merge_stream_shards([s[3] for s in shards], S)
         assert torch.equal(merged, full.tokens), t
+        check_tokens_against_oracle(wl, t, merged.cpu().numpy())      # and not only equal to another CUDA context
     # a frame needs every stream: sharded contexts refuse frame emission
     fr = torch.zeros((R, shards[1][3].shape[1]), dtype=torch.int32, device=dev)
     dl = torch.zeros((R, 16, shards[1][3].shape[1]), dtype=torch.int32, device=dev)
@@ -363,6 +364,7 @@ def test_device_side_token_exchange_between_stream_shards(dev, world):
             assert torch.equal(rk["all"], full.tokens), (t, g)
             rc, row = rk["ctx"].last_device_error()
             assert rc == 0
+        check_tokens_against_oracle(wl, t, ranks[-1]["all"].cpu().numpy())     # the gathered matrix against the oracle itself
     # graph replay: the epochs live on the device
     sts = {t: wl.step(t).to(dev) for t in (10, 11)}
     g = torch.cuda.CUDAGraph()
@@ -386,10 +388,74 @@ def test_device_side_token_exchange_between_stream_shards(dev, world):
     # the exchange needs the global stream count, and there is one per context
     with pytest.raises(pkg.CfgmsError):
         ranks[0]["ctx"].exchange_create(world, 0)
+    # the binding hands the library exactly one block address per rank
+    with pytest.raises(ValueError):
+        ranks[0]["ctx"].exchange_connect([x["addr"] for x in ranks] + [ranks[0]["addr"]])
+    with pytest.raises(ValueError):
+        ranks[0]["ctx"].exchange_connect_ipc([b"\0" * 64] * (world + 1))
+    # The request state advances on the PRIMARY stream's token: the rank that holds global stream 0 writes it (and
+    # writes what the unsharded context writes); a rank without that stream is refused instead of silently leaving
+    # step_next_out / n_frames_next_out / done_out untouched.
+    st = wl.step(8).to(dev)
+    mk = lambda: torch.full((R,), -9, dtype=torch.int32, device=dev)
+    want = [mk(), mk(), mk()]
+    full.ctx.step(full.hidden(8), full.pair_map, full.w, full.temp, full.top_k, wl.seed, st, full.tokens, req_id=full.req_id,
+                  n_frames=full.n_frames, eos_token=3, step_next_out=want[0], n_frames_next_out=want[1], done_out=want[2])
+    have = [mk(), mk(), mk()]
+    ranks[0]["ctx"].step(full.hidden(8), full.pair_map, full.w, full.temp, full.top_k, wl.seed, st, ranks[0]["tok"],
+                         req_id=full.req_id, n_frames=full.n_frames, eos_token=3, step_next_out=have[0],
+                         n_frames_next_out=have[1], done_out=have[2])
+    torch.cuda.synchronize()
+    for a, b in zip(want, have):
+        assert torch.equal(a, b) and bool((a.cpu().numpy()[wl.head_rows()] != -9).all())
+    for rk in ranks[1:]:
+        for kw in (dict(step_next_out=mk()), dict(n_frames_next_out=mk()), dict(done_out=mk())):
+            with pytest.raises(pkg.CfgmsError) as e:
+                rk["ctx"].step(full.hidden(8), full.pair_map, full.w, full.temp, full.top_k, wl.seed, st, rk["tok"],
+                               req_id=full.req_id, n_frames=full.n_frames, **kw)
+            assert e.value.status == 1      # CFGMS_ERR_ARG
     if world > 1:
         lone = pkg.Context(ranks[1]["heads"], ranks[1]["embeds"], max_rows=R, stream_base=1, stream_stride=world)
         with pytest.raises(pkg.CfgmsError):
             lone.exchange_create(world, 1)
         lone.close()
     for rk in ranks:
+        rk["ctx"].close()
+
+
+def test_exchange_wait_timeout_is_latched_and_the_context_survives(dev):
+    """A peer that has not stepped yet: the wait gives up after its 2 s bound, latches CFGMS_ERR_TIMEOUT in the sticky
+    error word and leaves the gathered tokens and its step count alone — no trap, the CUDA context stays usable — so
+    the same step can be waited for again once the late peer has delivered."""
+    import paper_2607_02119_b200 as pkg
+    from paper_2607_02119_b200 import dist_utils
+    wl = _custom(pairs=3, singles=2, d=128, S=4, V=128, T=16, mixed=True)
+    full = DeviceWorkload(wl, dev)
+    R, S = wl.R, wl.S
+    ranks = []
+    for g in range(2):
+        base, stride, s_local = dist_utils.stream_shard(g, 2, S)
+        heads = wl.heads[base::stride].contiguous().to(dev)
+        embeds = wl.embeds[base::stride].contiguous().to(dev)
+        ctx = pkg.Context(heads, embeds, max_rows=R, stream_base=base, stream_stride=stride, global_streams=S)
+        _, addr = ctx.exchange_create(2, g)
+        ranks.append(dict(ctx=ctx, heads=heads, embeds=embeds, addr=addr, tok=torch.full((R, s_local), -1, dtype=torch.int32, device=dev)))
+    for rk in ranks:
+        rk["ctx"].exchange_connect([x["addr"] for x in ranks])
+    st = wl.step(6).to(dev)
+    step = lambda rk: rk["ctx"].step(full.hidden(6), full.pair_map, full.w, full.temp, full.top_k, wl.seed, st, rk["tok"],
+                                     req_id=full.req_id, n_frames=full.n_frames)
+    step(ranks[0])
+    ranks[0]["ctx"].exchange_wait(R)               # rank 1 has not stepped: 2 s, then the latch
+    torch.cuda.synchronize()                       # a trap would surface here as a CUDA error
+    assert ranks[0]["ctx"].last_device_error() == (7, 11)      # CFGMS_ERR_TIMEOUT, raised by the wait kernel
+    assert ranks[0]["ctx"].last_device_error()[0] == 0
+    step(ranks[1])                                 # the late peer delivers
+    for rk in ranks:
+        rk["ctx"].exchange_wait(R)
+    full.step(6)
+    torch.cuda.synchronize()
+    for rk in ranks:
+        assert rk["ctx"].last_device_error()[0] == 0
+        assert torch.equal(rk["ctx"].exchange_tokens(R, S), full.tokens)
         rk["ctx"].close()
