@@ -20,12 +20,21 @@ FLAG_INACTIVE, FLAG_GREEDY, FLAG_CLOSE, FLAG_BOUNDARY, FLAG_FORCED = 1, 2, 4, 8,
 TOL = 2e-2  # north_star's margin below which a tie is "close" (counted, not failed)
 
 
+# CFGMS_ORACLE_SANITIZE=1 (tests/test_oracle_sanitizers.py sets it for a child process that preloads the ASan
+# runtime): the same source built with AddressSanitizer + UndefinedBehaviorSanitizer into a library of its own.
+_SANITIZE = os.environ.get("CFGMS_ORACLE_SANITIZE", "") == "1"
+if _SANITIZE:
+    _LIB = os.path.join(_HERE, "liboracle_san.so")
+
+
 def build(force: bool = False) -> str:
     """gcc -O2, no fast-math, no FMA contraction: the fp64 sums keep the written order."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-               "-o", _LIB, _SRC, "-lm"]
-        subprocess.run(cmd, check=True)
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off"]
+        if _SANITIZE:   # same arithmetic (no contraction, same order); -O1 and frame pointers for readable reports
+            cmd = ["gcc", "-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                   "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off"]
+        subprocess.run(cmd + ["-o", _LIB, _SRC, "-lm"], check=True)
     return _LIB
 
 

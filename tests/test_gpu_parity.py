@@ -409,10 +409,10 @@ def test_overlap_counters_survive_steps_whose_cells_are_mostly_pad(dev):
     ov.check_no_device_error()
 
 
-@pytest.mark.parametrize("cfg,n_cells", [(5, 96), (3, 64), (2, 256)])
+@pytest.mark.parametrize("cfg,n_cells", [(5, 96), (4, 96), (3, 64), (2, 256)])
 def test_bench_launch_configuration_graph_replay(dev, cfg, n_cells):
     """The launch configuration bench.py times: default policy (config 5: lean GEMM + dependent finalize
-    beside it; configs 2-3: full-register GEMM, serial finalize), no debug tap, consecutive steps
+    beside it; configs 2-4: full-register GEMM, serial finalize), no debug tap, consecutive steps
     captured in ONE CUDA graph and replayed.  Tokens of every captured step are read back from the
     delayed buffer and compared with the oracle on a seeded sample of cells."""
     wl = workloads.make_config(cfg)
@@ -457,4 +457,6 @@ def test_bench_launch_configuration_graph_replay(dev, cfg, n_cells):
             else:
                 assert got == ref.tok[j], (t, c, i, got, ref.tok[j], ref.margin[j])
     print(f"config{cfg} graph replay: {n_sampled} sampled cells, close ties {n_close}, of which differ {n_mismatch}")
-    assert n_mismatch <= n_close <= CLOSE_FRAC_MAX * n_sampled + 2
+    # config 4 mixes in unpaired and greedy requests, whose un-extrapolated logits tie within 2e-2 several times more often
+    # (the two populations are counted apart, with this same 0.10 bound, in test_config4_mixed_continuous_batch)
+    assert n_mismatch <= n_close <= (0.10 if cfg == 4 else CLOSE_FRAC_MAX) * n_sampled + 2
