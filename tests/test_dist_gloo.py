@@ -136,3 +136,39 @@ def test_two_rank_exchange_handles_and_flag_protocol():
     flags = torch.zeros((world, world), dtype=torch.int64).share_memory_()
     mp.spawn(_exchange_worker_entry, args=(world, 29617, out, bufs, flags), nprocs=world, join=True)
     assert out[0] is True and out[1] is True
+
+
+def test_bench_spawns_its_own_ranks_when_asked_for_more_than_one_gpu():
+    """`python bench.py --gpus 2` typed WITHOUT torchrun must run two ranks (it re-launches itself the way the driver
+    launches it: one process per GPU, rendezvous on 127.0.0.1, a free port) and report n_gpus = 2.  --dry-ranks takes
+    the kernels out (gloo, no GPU) and keeps the plumbing: rendezvous, world == --gpus, barrier, the whole-job
+    reduction of the timed region (rank r 'serves' 10 requests in 1 + r ms -> 20 requests / 2 ms)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dry-ranks"], env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout                                   # rank 0 alone prints
+    assert lines[0]["n_gpus"] == 2 and lines[0]["worst_ms"] == 2.0 and lines[0]["value"] == 10000.0
+    # a world that does not match --gpus is an error, not a line that claims n_gpus = 1
+    bad = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dry-ranks"],
+                         env=dict(env, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0"), capture_output=True, text=True, timeout=120)
+    assert bad.returncode != 0 and "WORLD_SIZE" in (bad.stderr + bad.stdout)
+
+
+def test_bench_spawn_command_is_the_drivers_launch():
+    import importlib.util
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "7"], 12345)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "12345"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "7"] and cmd[-5].endswith("bench.py")
+    p = bench.free_port()
+    assert 1024 < p < 65536
