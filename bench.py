@@ -570,7 +570,8 @@ def main():
                     help="profiling aid: time the main graph and the kernels only (no e2e, no cpu baseline, no regimes); "
                          "the line then lacks those keys and is not a bench record")
     ap.add_argument("--probes", action="store_true",
-                    help="also time the two measurement probes (noise drawn in the GEMM epilogue; no logit spill) at configs 2, 3, 5")
+                    help="also time the two measurement probes (noise drawn in the GEMM epilogue; no logit spill) at configs 2, 3, 5; "
+                         "builds and loads the probe variant of the library (libcfgms_probes.so): not a bench record")
     ap.add_argument("--cta-pair", default="auto", choices=["auto", "on", "off"],
                     help="tuning: force the CTA-pair (cta_group::2) or the one-CTA head GEMM")
     ap.add_argument("--dry-ranks", action="store_true",
@@ -595,6 +596,11 @@ def main():
     import torch
     from paper_2607_02119_b200 import dist_utils
     import paper_2607_02119_b200 as pkg
+    if args.probes:
+        # the probes are compiled only into a separate measurement build of the library; the WHOLE run then uses it,
+        # so a --probes line is a design-choice measurement, never the bench record
+        from paper_2607_02119_b200 import binding, build
+        binding.use_library(build.build_lib(probes=True))
     pkg.library()  # fail loudly before anything else if the CUDA library is missing
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -651,7 +657,7 @@ def main():
                                    wl.n_req * wl.S * wl.V * 4 / 2 ** 20),
                                row_tile=info["row_tile"], row_blocks=info["row_blocks"], gemm_grid=info["gemm_grid"],
                                pipeline_stages=info["pipeline_stages"], cta_pair=bool(info["cta_pair"]), split_k=info["split_k"]),
-                "clocks": sampler.summary(), "gpu_launches": int((info["launches_last_step"] + (1 if sharded else 0)) * K + (0 if sharded else 1)),
+                "library": pkg.version(), "clocks": sampler.summary(), "gpu_launches": int((info["launches_last_step"] + (1 if sharded else 0)) * K + (0 if sharded else 1)),
                 "roofline": roof}
 
     if args.quick:

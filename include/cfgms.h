@@ -77,13 +77,6 @@ typedef enum { CFGMS_BF16 = 0, CFGMS_F32 = 1 } cfgms_dtype;
                                     distributed shared memory; the default whenever the (vocabulary tile pair,
                                     128-row block) tiles fill at most a quarter of the SMs)                   */
 
-/* Measurement probes behind DESIGN.md section 7's two argued design choices; never part of a product run. */
-#define CFGMS_CFG_PROBE_EPILOGUE_NOISE 256u /* the head GEMM's epilogue additionally draws the Philox-Gumbel noise of
-                                    EVERY merged logit (the literal "noise fused into the epilogue"); the draws are
-                                    discarded, tokens are unchanged: a lower bound of that variant's cost           */
-#define CFGMS_CFG_PROBE_NO_SPILL 512u /* the head GEMM does not write the fp32 logit spill (timing only: cells whose
-                                    sampling needs a spilled row are then wrong)                                 */
-
 typedef struct {
     int32_t max_rows;  /* largest R accepted by cfgms_step; <= 0 means 1024                     */
     int32_t pad_token; /* written at inactive (step, stream) cells when CFGMS_CFG_PAD_TOKEN      */

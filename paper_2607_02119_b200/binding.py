@@ -21,8 +21,6 @@ CFGMS_CFG_NO_OVERLAP = 16
 CFGMS_CFG_OVERLAP = 32
 CFGMS_CFG_NO_PDL_FINALIZE = 64
 CFGMS_CFG_NO_SPLIT_K = 128
-CFGMS_CFG_PROBE_EPILOGUE_NOISE = 256
-CFGMS_CFG_PROBE_NO_SPILL = 512
 CFGMS_FRAMES_UNSET = 2 ** 31 - 1
 
 STATUS = {0: "CFGMS_OK", 1: "CFGMS_ERR_ARG", 2: "CFGMS_ERR_SHAPE", 3: "CFGMS_ERR_LAYOUT", 4: "CFGMS_ERR_CUDA",
@@ -137,6 +135,15 @@ def library():
     return _lib()
 
 
+def use_library(path: str) -> None:
+    """Load another build of the library instead of libcfgms.so — the probe build of `bench.py --probes`
+    (build.build_lib(probes=True)).  Must be called before the first library call of the process."""
+    global LIB_PATH
+    if _LIB is not None:
+        raise RuntimeError("the library is already loaded")
+    LIB_PATH = path
+
+
 def version() -> str:
     return _lib().cfgms_version().decode()
 
@@ -223,7 +230,9 @@ class Context:
             cfg.flags |= CFGMS_CFG_NO_PDL_FINALIZE
         if no_split_k:             # tuning: never run a one-wave head GEMM as split-K clusters
             cfg.flags |= CFGMS_CFG_NO_SPLIT_K
-        cfg.flags |= int(probe) & (CFGMS_CFG_PROBE_EPILOGUE_NOISE | CFGMS_CFG_PROBE_NO_SPILL)   # measurement probes (bench.py --probes)
+        # measurement probes (bench.py --probes): two flag bits only the probe build of the library knows (use_library);
+        # the product library answers them with CFGMS_ERR_ARG
+        cfg.flags |= int(probe) & 0x300
         self.pad_token = self.V if pad_token is None else int(pad_token)
         h = C.c_void_p()
         with torch.cuda.device(heads.device):

@@ -19,6 +19,12 @@
 
 using namespace cfgms;
 
+// Measurement probes are not part of the C ABI: the two flag bits exist only in the probe build
+// (`python -m paper_2607_02119_b200.build --probes` -> libcfgms_probes.so, used by `bench.py --probes`).  The product
+// build refuses them, so that a probe run against the wrong library fails instead of timing the product path.
+#define CFGMS_CFG_PROBE_EPILOGUE_NOISE 256u /* the head GEMM's epilogue also draws the Philox-Gumbel noise of EVERY merged logit */
+#define CFGMS_CFG_PROBE_NO_SPILL 512u       /* the head GEMM does not write the fp32 logit spill (timing only: wrong tokens)    */
+
 namespace {
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -56,7 +62,9 @@ struct cfgms_ctx {
     int split_mode = 0;               // split-K for one-wave GEMMs: 0 = chosen per step, 1 = never
     int max_clusters4 = 0;            // four-CTA clusters of the split-K kernel that can be co-resident on this device
     bool pdl_finalize = true;         // serial mode: launch a small K2 grid as a programmatic dependent of K1
+#ifdef CFGMS_PROBES
     int probe = 0;                    // measurement probes (CFGMS_CFG_PROBE_*), see GemmParams::probe
+#endif
     const __nv_bfloat16* heads = nullptr;
     float* bias = nullptr;            // [NT] what the epilogue adds: bias_base (+ the caller's logit bias)
     float* bias_base = nullptr;       // [NT] W_i e_i, folded at create
@@ -203,7 +211,11 @@ const char* cfgms_strerror(int s) {
     }
 }
 
+#ifdef CFGMS_PROBES
+const char* cfgms_version(void) { return "cfgms 0.1 sm_100a (tcgen05/TMEM/TMA) +probes (measurement build, not the product), built " __DATE__; }
+#else
 const char* cfgms_version(void) { return "cfgms 0.1 sm_100a (tcgen05/TMEM/TMA), built " __DATE__; }
+#endif
 
 int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t S, int32_t d, int32_t V,
                  const cfgms_config* cfg) {
@@ -270,7 +282,11 @@ int cfgms_create(cfgms_ctx** out, const void* heads, const void* embeds, int32_t
     c->overlap_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_OVERLAP)) ? 1 : (cfg && (cfg->flags & CFGMS_CFG_OVERLAP)) ? 2 : 0;
     c->pdl_finalize = !(cfg && (cfg->flags & CFGMS_CFG_NO_PDL_FINALIZE));
     c->split_mode = (cfg && (cfg->flags & CFGMS_CFG_NO_SPLIT_K)) ? 1 : 0;
+#ifdef CFGMS_PROBES
     c->probe = (cfg && (cfg->flags & CFGMS_CFG_PROBE_EPILOGUE_NOISE) ? 1 : 0) | (cfg && (cfg->flags & CFGMS_CFG_PROBE_NO_SPILL) ? 2 : 0);
+#else
+    if (cfg && (cfg->flags & (CFGMS_CFG_PROBE_EPILOGUE_NOISE | CFGMS_CFG_PROBE_NO_SPILL))) { cfgms_destroy(c); return CFGMS_ERR_ARG; }
+#endif
     c->overlap = c->use_cand && (V % kBM) == 0 && c->overlap_mode != 1;
     if (c->overlap) {
         c->ready_words = ((S * ((c->max_rows + 63) / 64) + 1 + 1) & ~1) + 32;   // counters | done | pad | stats (16 x u64)
@@ -451,7 +467,9 @@ int step_impl(cfgms_ctx* c, const cfgms_step_args* a, cudaStream_t st, const Hos
     const bool overlap = !up && !split && c->overlap && (c->overlap_mode == 2 || gp.num_tiles >= kOverlapMinWaves * workers);
     gp.ready = overlap ? c->ready : nullptr;
     gp.V = c->V;
+#ifdef CFGMS_PROBES
     gp.probe = c->probe; gp.probe_sink = reinterpret_cast<uint32_t*>(c->err + 1);
+#endif
     gp.split_tma = gp.num_tiles < kOverlapMinWaves * workers ? 1 : 0;
     gp.split_k = split ? 2 : 1;
     // weights are streamed (read by one CTA when there is a single row block) — unless the whole head is small enough to

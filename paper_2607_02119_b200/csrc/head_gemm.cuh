@@ -36,7 +36,7 @@
 // the GEMM is still running.
 #pragma once
 #include "ptx_sm100.cuh"
-#include "finalize.cuh"   // gumbel_noise (the epilogue-noise measurement probe below)
+#include "finalize.cuh"   // gumbel_noise (the epilogue-noise measurement probe of the -DCFGMS_PROBES build)
 
 namespace cfgms {
 
@@ -82,13 +82,17 @@ struct GemmParams {
     int V;               // tokens per stream (ready != nullptr requires V % kBM == 0)
     int split_tma;       // 1: warp 2 issues the row-tile loads; 0: warp 0 issues both (warp 2 idles)
     int split_k;         // 1, or 2: one-wave GEMMs run on four-CTA clusters, two CTA pairs each taking half of K (kSplit build)
-    // Measurement probes for the two design choices DESIGN.md section 7 argues (never set by default):
+#ifdef CFGMS_PROBES
+    // Measurement probes for the two design choices DESIGN.md section 7 argues.  They exist only in the probe build of
+    // the library (-DCFGMS_PROBES, libcfgms_probes.so, `bench.py --probes`); the product build has neither the fields
+    // nor the code:
     //   probe bit 0: draw the Philox-Gumbel noise of EVERY merged logit in this epilogue (north_star's literal
     //                fusion) — the draws are folded into a sink word, results are unchanged: a lower bound of what
     //                the fused variant costs;
     //   probe bit 1: do not write the z spill (timing only: cells that need a spilled row sample garbage).
     int probe;
     uint32_t* probe_sink;
+#endif
     uint64_t policy_w, policy_h;
 #ifdef CFGMS_TRACE
     unsigned long long* trace;
@@ -202,7 +206,11 @@ __device__ __forceinline__ void finish_slab(const GemmParams& p, const uint32_t 
     char* zp = reinterpret_cast<char*>(p.z + static_cast<size_t>(row_base) * NT + n);
     float* tp = kTap ? p.tap + static_cast<size_t>(row_base) * NT + n : nullptr;
     const size_t row_stride = 2 * NT * sizeof(float);         // bytes between the even rows of two slots
+#ifdef CFGMS_PROBES
     const bool spill = n_ok && !(p.probe & 2);
+#else
+    const bool spill = n_ok;
+#endif
     const int o = lane & 15, part = lane >> 4;                // candidate pass: request o of the warp's 16, token half `part`
     int any_kind = 0;
 #pragma unroll
@@ -222,6 +230,7 @@ __device__ __forceinline__ void finish_slab(const GemmParams& p, const uint32_t 
             if (kTap && own && n_ok) { const SlotCoefB t = cb[j]; tp[static_cast<size_t>(2 * j) * NT] = fmaf(t.m00, a0, fmaf(t.m01, a1, bias)); }
             if (kCand) stg[j * kStgPitch + lane] = (own && n_ok) ? z0 + 0.0f : -INFINITY;
         }
+#ifdef CFGMS_PROBES
         if (kCand && (p.probe & 1)) {
             // measurement probe: the noise of every merged logit of the slab, drawn here (rolled loop over the staged z
             // values so that the product path's code stays as it is); the draws are folded into a sink word
@@ -232,6 +241,7 @@ __device__ __forceinline__ void finish_slab(const GemmParams& p, const uint32_t 
                                         gumbel_noise(0x1234u, 0x5678u, static_cast<uint32_t>(row_base + 2 * j), 7, n >> 11, n & 2047));
             if (sink == 0x9e3779b9u) *p.probe_sink = sink;    // keeps the draws alive
         }
+#endif
         if (kCand) {
             __syncwarp();
             float val[4]; uint32_t src;

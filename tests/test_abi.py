@@ -27,6 +27,17 @@ def test_library_builds_and_exports_header_symbols():
     assert set(pkg.EXPORTS) == set(names)
 
 
+def test_measurement_probes_are_not_part_of_the_abi():
+    """The design-choice probes (one of which produces wrong tokens by design) live in a separate build of the
+    library (-DCFGMS_PROBES), not in the public header, the binding's constants or the product library's strings."""
+    import paper_2607_02119_b200 as pkg
+    from paper_2607_02119_b200 import binding
+    header = open(os.path.join(ROOT, "include", "cfgms.h")).read()
+    assert "PROBE" not in header
+    assert not [n for n in dir(binding) if "PROBE" in n]
+    assert "probes" not in pkg.version()
+
+
 def test_version_and_strerror_strings():
     import paper_2607_02119_b200 as pkg
     assert "sm_100a" in pkg.version()

@@ -323,6 +323,10 @@ def test_errors_are_reported_not_fatal(dev):
     assert rc == 3 and row == 0       # CFGMS_ERR_LAYOUT at the slot's even row
     assert dw.ctx.last_device_error()[0] == 0          # sticky word cleared
     # host-side validation
+    for bits in (256, 512):           # the measurement probes' flag bits: only the probe build of the library knows them
+        with pytest.raises(pkg.CfgmsError) as e:
+            pkg.Context(dw.heads, dw.embeds, max_rows=4, probe=bits)
+        assert e.value.status == 1
     small = pkg.Context(dw.heads, dw.embeds, max_rows=4)
     with pytest.raises(pkg.CfgmsError) as e:
         small.step(dw.hidden(0), dw.pair_map, dw.w, dw.temp, dw.top_k, 0, wl.step(0).to(dev), dw.tokens)
