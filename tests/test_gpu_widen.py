@@ -170,6 +170,11 @@ def _bf16_ulp(x):
     dict(R=7, S=3, V_e=50, d=64),            # odd row count, one 16-byte chunk per 8 columns
     dict(R=64, S=9, V_e=257, d=2048),        # OpusLM-like 9 streams
     dict(R=256, S=16, V_e=2049, d=4096),     # config-5 head shape (V + 1 rows: PAD has an embedding)
+    dict(R=9, S=20, V_e=33, d=1096),         # more streams than one round of gathers holds; a ragged column count
+    dict(R=1, S=64, V_e=5, d=8),             # one row, the most streams the head takes, one chunk
+    dict(R=33, S=20, V_e=33, d=1096),        # odd row count, three rounds of gathers, a slot whose rows differ
+    dict(R=40, S=64, V_e=9, d=512),          # the most streams the head takes, many rows
+    dict(R=700, S=3, V_e=11, d=4096),        # more slots than two waves of CTAs, few streams, wide rows
 ])
 def test_feedback_is_the_correctly_rounded_sum(dev, shape):
     R, S, V_e, d = shape["R"], shape["S"], shape["V_e"], shape["d"]
